@@ -1,0 +1,112 @@
+/* kappagen.h -- C ABI of libkappagen: the hot path of arXiv 2602.05606 (Zenitani & Umeda,
+ * "An approximate Kappa generator for particle simulations") for NVIDIA B200 (sm_100a).
+ *
+ * The operation (paper Table I; Eqs. (22)-(25)).  For the
+ * particle with global index g = offset + i:
+ *   (w0,w1,w2,w3) = Philox4x32-10(counter = (lo32 g, hi32 g, 0, 0), key = (lo32 seed, hi32 seed))
+ *   U1,U2,U3 = (w0+1/2)/2^32, (w1+1/2)/2^32, (w2+1/2)/2^32        "generate U1,U2,U3 ~ Uniform(0,1)"
+ *   L  = -kappa* {(1 - U1^(2/3))^(-1/kappa*) - 1}                  Eq. (25)
+ *   V  = theta sqrt(x),  x = positive root of b x^2 + (a + cL) x + L = 0      Eq. (24)
+ *   vx = V (2U2-1);  vy = 2V sqrt(U2(1-U2)) cos(2 pi U3);  vz = 2V sqrt(U2(1-U2)) sin(2 pi U3)
+ * with kappa* = kappa - 1/2, a, b, c from Table I lines 1-4 (Eqs. (16),(13),(17),(20)).
+ * The output is a pure function of the arguments: independent of launch shape, of chunking
+ * through `offset`, and of how many GPUs share the index range.
+ *
+ * Conventions for every call:
+ *  - "device" pointers are CUDA device memory owned by the caller (e.g. torch tensor.data_ptr());
+ *    "host" pointers are ordinary host memory.  The library keeps no state and no RNG state,
+ *    and allocates nothing that outlives a call.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device-buffer
+ *    calls enqueue on `stream` and return without synchronising; argument errors are returned
+ *    at once, asynchronous CUDA errors surface at the caller's next synchronisation.
+ *  - Output planes are SoA: vx[i], vy[i], vz[i]; element type float (KAPPAGEN_F32) or double
+ *    (KAPPAGEN_F64).  Planes must be aligned to the element size; 16-byte aligned planes take
+ *    the vector-store path, others a scalar-store path that writes the same values.
+ *  - Return value: KAPPAGEN_OK (0) or a negative kappagen_status.  kappagen_last_error()
+ *    returns a thread-local, human-readable description of the last failure.
+ *  - n == 0 (or ncell == 0, ppc == 0) is KAPPAGEN_OK and launches nothing.
+ */
+#ifndef KAPPAGEN_H_
+#define KAPPAGEN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { KAPPAGEN_F32 = 0, KAPPAGEN_F64 = 1 } kappagen_dtype;
+
+typedef enum {
+    KAPPAGEN_OK = 0,
+    KAPPAGEN_EINVAL = -1,     /* kappa <= 3/2, theta < 0, non-finite, n < 0, bad dtype, bad stride */
+    KAPPAGEN_ENULL = -2,      /* a required pointer is NULL while there is work to do               */
+    KAPPAGEN_EALIGN = -3,     /* a plane is not aligned to its element size                         */
+    KAPPAGEN_EWORKSPACE = -4, /* workspace NULL or smaller than kappagen_cells_workspace_bytes()    */
+    KAPPAGEN_ECUDA = -5       /* a CUDA runtime call or the launch failed                           */
+} kappagen_status;
+
+/* Table I lines 5-10 with uniform parameters (S1-S6 of DESIGN.md).
+ * n >= 0 particles; kappa > 3/2, theta >= 0 (theta == 0 writes zeros); particle i
+ * uses counter offset + i (64-bit, wraps).  vx, vy, vz: device, [n] elements of `dtype`. */
+int kappagen_sample(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                    int dtype, void* vx, void* vy, void* vz, void* stream);
+
+/* Same generator with PIC-style per-cell parameters ("10^2-10^3 particles in a grid cell",
+ * PAPER.md:215).  Cell-major: particle g = cell*ppc + j (0 <= j < ppc) uses counter offset + g,
+ * kappa[cell], theta[cell]; the cell's drift velocity is added last, in the output type.
+ *  kappa, theta : device, [ncell] elements of `dtype`.  A cell with kappa <= 3/2, theta < 0 or a
+ *                 non-finite value gets NaN in all its particles (it cannot be reported synchronously).
+ *  drift        : device, elements of `dtype`, or NULL (no drift).  drift_stride == 0: one shared
+ *                 (dx,dy,dz) at drift[0..2]; drift_stride == 1: per cell at drift[3*cell + 0..2].
+ *  workspace    : device scratch of at least kappagen_cells_workspace_bytes(ncell, dtype) bytes,
+ *                 16-byte aligned; holds the per-cell Table I lines 1-4 (computed on the device in
+ *                 double by a small pre-kernel on the same stream).  Contents are unspecified after.
+ *  vx, vy, vz   : device, [ncell*ppc] elements of `dtype`. */
+int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                          const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                          int dtype, void* vx, void* vy, void* vz,
+                          void* workspace, size_t workspace_bytes, void* stream);
+size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype);
+
+/* Host-buffer variant of kappagen_sample (the end-to-end path): vx, vy, vz are HOST arrays of
+ * [n] elements (pinned memory makes the copies asynchronous and fast; pageable memory works).
+ * Generates on the current device in chunks, double-buffered so that the device-to-host copy of
+ * one chunk overlaps the kernel of the next; allocates its staging buffers, frees them, and
+ * returns only when the host arrays are complete (synchronous).  Same values as kappagen_sample. */
+int kappagen_sample_host(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                         int dtype, void* vx_host, void* vy_host, void* vz_host);
+
+/* GPU baseline, NOT the paper's method: the "standard method" it is compared with (PAPER.md:17,
+ * :180, :219-224): v = theta sqrt(kappa/(2g)) (n1,n2,n3), n_j ~ N(0,1) by Box-Muller, g ~
+ * Gamma(kappa-1/2) by the Marsaglia-Tsang rejection loop.  Samples the EXACT Kappa distribution;
+ * validated statistically only.  Same output contract as kappagen_sample.  trip_counters
+ * (device, 2 x uint64, optional, caller zeroes it): [0] += sum over lanes of loop trips,
+ * [1] += sum over warps of 32 x (trips of the slowest lane), to compare with Eq. (30). */
+int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                         int dtype, void* vx, void* vy, void* vz, void* stream,
+                         unsigned long long* trip_counters);
+
+/* Test hook for the "uniforms bit-exact" gate: the Philox words particle i consumes, produced by
+ * the same device function the samplers call.  w0, w1, w2: device, [n] uint32 each. */
+int kappagen_words(int64_t n, uint64_t seed, uint64_t offset,
+                   uint32_t* w0, uint32_t* w1, uint32_t* w2, void* stream);
+
+/* Test hook: velocities from caller-chosen words instead of Philox (same device math as
+ * kappagen_sample, S2-S6), so parity can be driven through the extreme words.  w0,w1,w2: device. */
+int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                               double kappa, double theta, int dtype,
+                               void* vx, void* vy, void* vz, void* stream);
+
+/* Table I lines 1-4 on the host in double, exactly as kappagen_sample computes them before launch.
+ * All four outputs are host pointers and required. */
+int kappagen_params(double kappa, double* kappa_star, double* a, double* b, double* c);
+
+const char* kappagen_last_error(void);
+int kappagen_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KAPPAGEN_H_ */

@@ -1,0 +1,319 @@
+// kappagen_api.cu -- the C ABI of include/kappagen.h: argument checks and kernel launches.
+// Every step of the hot path runs in the kernels of kernels.cuh; nothing here computes a velocity,
+// and there is no CPU fallback: without a CUDA device the calls return KAPPAGEN_ECUDA.
+#include <cstdint>
+#include <cstdio>
+#include <cuda_runtime.h>
+
+#include "../../include/kappagen.h"
+#include "baseline_mt.cuh"
+#include "host_params.hpp"
+#include "kernels.cuh"
+
+namespace kappagen {
+
+#define KG_CUDA(call)                                                                    \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            set_error("%s: %s failed: %s", __func__, #call, cudaGetErrorString(e_));     \
+            return KAPPAGEN_ECUDA;                                                       \
+        }                                                                                \
+    } while (0)
+
+static inline bool aligned_to(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+static inline size_t elem_size(int dtype) { return dtype == KAPPAGEN_F32 ? 4 : 8; }
+
+// Grid for a grid-stride kernel: enough blocks to fill every SM at the kernel's occupancy, never more
+// than there are tiles.  `blocks_per_sm` comes from the occupancy API, once per kernel and device.
+template <typename Kernel>
+static int grid_for(Kernel kernel, int64_t tiles, int* grid_out) {
+    int dev = 0, sms = 0, per_sm = 0;
+    KG_CUDA(cudaGetDevice(&dev));
+    KG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    KG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0));
+    if (per_sm < 1) per_sm = 1;
+    const int64_t full = (int64_t)sms * per_sm;
+    *grid_out = (int)(tiles < full ? tiles : full);
+    return KAPPAGEN_OK;
+}
+
+static int check_planes(const char* fn, int64_t n, int dtype, const void* vx, const void* vy, const void* vz,
+                        bool* vec) {
+    if (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64) {
+        set_error("%s: dtype %d is neither KAPPAGEN_F32 nor KAPPAGEN_F64", fn, dtype);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n < 0) {
+        set_error("%s: negative particle count %lld", fn, (long long)n);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!vx || !vy || !vz) {
+        set_error("%s: NULL output plane", fn);
+        return KAPPAGEN_ENULL;
+    }
+    const size_t es = elem_size(dtype);
+    if (!aligned_to(vx, es) || !aligned_to(vy, es) || !aligned_to(vz, es)) {
+        set_error("%s: output plane not aligned to its element size (%zu)", fn, es);
+        return KAPPAGEN_EALIGN;
+    }
+    *vec = aligned_to(vx, 16) && aligned_to(vy, 16) && aligned_to(vz, 16);
+    return KAPPAGEN_OK;
+}
+
+template <typename T>
+static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, bool vec,
+                         T* vx, T* vy, T* vz, cudaStream_t st) {
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    const int64_t tiles = (n + tile - 1) / tile;
+    int grid = 0, rc;
+    if (vec) {
+        if ((rc = grid_for(sample_kernel<T, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        sample_kernel<T, true><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
+    } else {
+        if ((rc = grid_for(sample_kernel<T, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        sample_kernel<T, false><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
+    }
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+static int sample_on_stream(const char* fn, int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                            int dtype, void* vx, void* vy, void* vz, cudaStream_t st) {
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    const PhiloxKeys K = philox_expand_keys(seed);
+    if (dtype == KAPPAGEN_F32)
+        return launch_sample<float>(n, offset, K, host_coef_f32(kappa, theta), vec, (float*)vx, (float*)vy, (float*)vz, st);
+    return launch_sample<double>(n, offset, K, host_coef_f64(kappa, theta), vec, (double*)vx, (double*)vy, (double*)vz, st);
+}
+
+template <typename T>
+static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift,
+                        int64_t drift_stride, uint64_t offset, const PhiloxKeys& K, bool vec, T* vx, T* vy, T* vz,
+                        Coef<T>* W, cudaStream_t st) {
+    const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
+    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, W);
+    KG_CUDA(cudaGetLastError());
+    const int64_t n = ncell * (int64_t)ppc;
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    const int64_t tiles = (n + tile - 1) / tile;
+    int grid = 0, rc;
+    if (vec) {
+        if ((rc = grid_for(sample_cells_kernel<T, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        sample_cells_kernel<T, true><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, offset, K, W, drift, drift_stride, vx, vy, vz);
+    } else {
+        if ((rc = grid_for(sample_cells_kernel<T, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        sample_cells_kernel<T, false><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, offset, K, W, drift, drift_stride, vx, vy, vz);
+    }
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+template <typename T>
+static int launch_mt(int64_t n, double kappa, double theta, uint64_t offset, const PhiloxKeys& K, T* vx, T* vy,
+                     T* vz, unsigned long long* trips, cudaStream_t st) {
+    MtParams<T> P;
+    const double d = (kappa - 0.5) - 1.0 / 3.0;
+    P.d = (T)d;
+    P.cp = (T)(1.0 / sqrt(9.0 * d));
+    P.scale = (T)(theta * sqrt(0.5 * kappa));
+    int grid = 0, rc;
+    if ((rc = grid_for(baseline_mt_kernel<T>, (n + kThreads - 1) / kThreads, &grid)) != KAPPAGEN_OK) return rc;
+    baseline_mt_kernel<T><<<grid, kThreads, 0, st>>>(n, offset, K, P, vx, vy, vz, trips);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+}  // namespace kappagen
+
+using namespace kappagen;
+
+extern "C" int kappagen_sample(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                               void* vx, void* vy, void* vz, void* stream) {
+    return sample_on_stream("kappagen_sample", n, kappa, theta, seed, offset, dtype, vx, vy, vz, (cudaStream_t)stream);
+}
+
+extern "C" size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype) {
+    if (ncell <= 0 || (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64)) return 0;
+    return (size_t)ncell * (dtype == KAPPAGEN_F32 ? sizeof(Coef<float>) : sizeof(Coef<double>));
+}
+
+extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                     const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                     int dtype, void* vx, void* vy, void* vz, void* workspace,
+                                     size_t workspace_bytes, void* stream) {
+    const char* fn = "kappagen_sample_cells";
+    if (ncell < 0 || ppc < 0) {
+        set_error("%s: negative ncell or ppc", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (ncell > 0 && ppc > 0 && ncell > INT64_MAX / ppc) {
+        set_error("%s: ncell*ppc overflows", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    bool vec = false;
+    const int64_t n = ncell * (int64_t)ppc;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (drift != nullptr && drift_stride != 0 && drift_stride != 1) {
+        set_error("%s: drift_stride must be 0 (shared) or 1 (per cell), got %lld", fn, (long long)drift_stride);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!kappa || !theta) {
+        set_error("%s: NULL kappa or theta array", fn);
+        return KAPPAGEN_ENULL;
+    }
+    const size_t es = elem_size(dtype);
+    if (!aligned_to(kappa, es) || !aligned_to(theta, es) || (drift && !aligned_to(drift, es))) {
+        set_error("%s: kappa/theta/drift not aligned to the element size", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    if (!workspace || workspace_bytes < kappagen_cells_workspace_bytes(ncell, dtype) || !aligned_to(workspace, 16)) {
+        set_error("%s: workspace NULL, misaligned or smaller than %zu bytes", fn, kappagen_cells_workspace_bytes(ncell, dtype));
+        return KAPPAGEN_EWORKSPACE;
+    }
+    const PhiloxKeys K = philox_expand_keys(seed);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32)
+        return launch_cells<float>(ncell, ppc, (const float*)kappa, (const float*)theta, (const float*)drift, drift_stride,
+                                   offset, K, vec, (float*)vx, (float*)vy, (float*)vz, (Coef<float>*)workspace, st);
+    return launch_cells<double>(ncell, ppc, (const double*)kappa, (const double*)theta, (const double*)drift, drift_stride,
+                                offset, K, vec, (double*)vx, (double*)vy, (double*)vz, (Coef<double>*)workspace, st);
+}
+
+extern "C" int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                                    void* vx, void* vy, void* vz, void* stream, unsigned long long* trip_counters) {
+    const char* fn = "kappagen_baseline_mt";
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    const PhiloxKeys K = philox_expand_keys(seed);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32)
+        return launch_mt<float>(n, kappa, theta, offset, K, (float*)vx, (float*)vy, (float*)vz, trip_counters, st);
+    return launch_mt<double>(n, kappa, theta, offset, K, (double*)vx, (double*)vy, (double*)vz, trip_counters, st);
+}
+
+extern "C" int kappagen_words(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
+                              void* stream) {
+    const char* fn = "kappagen_words";
+    if (n < 0) {
+        set_error("%s: negative count", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!w0 || !w1 || !w2) {
+        set_error("%s: NULL output", fn);
+        return KAPPAGEN_ENULL;
+    }
+    if (!aligned_to(w0, 4) || !aligned_to(w1, 4) || !aligned_to(w2, 4)) {
+        set_error("%s: outputs must be 4-byte aligned", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    int grid = 0, rc;
+    if ((rc = grid_for(words_kernel, (n + kThreads - 1) / kThreads, &grid)) != KAPPAGEN_OK) return rc;
+    words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                          double kappa, double theta, int dtype, void* vx, void* vy, void* vz,
+                                          void* stream) {
+    const char* fn = "kappagen_velocity_of_words";
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!w0 || !w1 || !w2) {
+        set_error("%s: NULL word array", fn);
+        return KAPPAGEN_ENULL;
+    }
+    int grid = 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t tiles = (n + kThreads - 1) / kThreads;
+    if (dtype == KAPPAGEN_F32) {
+        if ((rc = grid_for(velocity_of_words_kernel<float>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        velocity_of_words_kernel<float><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f32(kappa, theta),
+                                                                   (float*)vx, (float*)vy, (float*)vz);
+    } else {
+        if ((rc = grid_for(velocity_of_words_kernel<double>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        velocity_of_words_kernel<double><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f64(kappa, theta),
+                                                                    (double*)vx, (double*)vy, (double*)vz);
+    }
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+// End-to-end path: host destination, chunked, double-buffered (the copy of chunk c overlaps the kernel
+// of chunk c+1 on the other stream).
+extern "C" int kappagen_sample_host(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                                    void* vx_host, void* vy_host, void* vz_host) {
+    const char* fn = "kappagen_sample_host";
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx_host, vy_host, vz_host, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    const size_t es = elem_size(dtype);
+    const int64_t chunk = n < ((int64_t)1 << 22) ? n : ((int64_t)1 << 22);   // 48 / 96 MiB of output per chunk
+    const size_t plane = (((size_t)chunk * es) + 255) & ~(size_t)255;
+    char* dev = nullptr;
+    cudaStream_t st[2] = {nullptr, nullptr};
+    KG_CUDA(cudaMalloc(&dev, 6 * plane));
+    int status = KAPPAGEN_OK;
+    for (int b = 0; b < 2 && status == KAPPAGEN_OK; ++b)
+        if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) {
+            set_error("%s: cudaStreamCreate failed", fn);
+            status = KAPPAGEN_ECUDA;
+        }
+    int64_t done = 0;
+    for (int c = 0; done < n && status == KAPPAGEN_OK; ++c) {
+        const int b = c & 1;
+        const int64_t m = (n - done) < chunk ? (n - done) : chunk;
+        char* d = dev + (size_t)b * 3 * plane;
+        status = sample_on_stream(fn, m, kappa, theta, seed, offset + (uint64_t)done, dtype, d, d + plane, d + 2 * plane, st[b]);
+        if (status != KAPPAGEN_OK) break;
+        char* hv[3] = {(char*)vx_host, (char*)vy_host, (char*)vz_host};
+        for (int q = 0; q < 3; ++q) {
+            if (cudaMemcpyAsync(hv[q] + (size_t)done * es, d + (size_t)q * plane, (size_t)m * es, cudaMemcpyDeviceToHost,
+                                st[b]) != cudaSuccess) {
+                set_error("%s: cudaMemcpyAsync failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
+                status = KAPPAGEN_ECUDA;
+            }
+        }
+        done += m;
+    }
+    for (int b = 0; b < 2; ++b) {
+        if (st[b]) {
+            if (cudaStreamSynchronize(st[b]) != cudaSuccess && status == KAPPAGEN_OK) {
+                set_error("%s: stream synchronize failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
+                status = KAPPAGEN_ECUDA;
+            }
+            cudaStreamDestroy(st[b]);
+        }
+    }
+    cudaFree(dev);
+    return status;
+}

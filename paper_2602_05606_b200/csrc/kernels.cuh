@@ -1,0 +1,162 @@
+// kernels.cuh -- the kappagen kernels (sm_100a).  Launchers and the C ABI are in kappagen_api.cu.
+//
+// Mapping.  A thread produces G = 16/sizeof(T) consecutive particles per group, so that each of its
+// three stores is one 128-bit st.global (a warp writes 512 contiguous bytes per plane), and NG groups
+// per tile for instruction-level parallelism.  Blocks walk the index range in a grid-stride loop; the
+// output is a pure function of the particle index, so the mapping never shows in the result.
+// The path is write-only: 0 bytes read, 3*sizeof(T) bytes written per particle (12 fp32 / 24 fp64).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "coefs.cuh"
+#include "math_f32.cuh"
+#include "math_f64.cuh"
+#include "philox.cuh"
+
+namespace kappagen {
+
+constexpr int kThreads = 256;
+constexpr int kGroups = 2;  // 128-bit groups per thread per tile
+
+template <typename T> struct Vec128;
+template <> struct Vec128<float> { using type = float4; };
+template <> struct Vec128<double> { using type = double2; };
+
+__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<float>& C,
+                                         float& x, float& y, float& z) { velocity_f32(w0, w1, w2, C, x, y, z); }
+__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<double>& C,
+                                         double& x, double& y, double& z) { velocity_f64(w0, w1, w2, C, x, y, z); }
+
+// Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
+__device__ __forceinline__ void store_group(float* p, const float (&v)[4]) {
+    __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
+}
+__device__ __forceinline__ void store_group(double* p, const double (&v)[2]) {
+    __stcs(reinterpret_cast<double2*>(p), make_double2(v[0], v[1]));
+}
+
+template <typename T, bool VEC, int G>
+__device__ __forceinline__ void store_planes(int64_t i, int64_t n, T* __restrict__ vx, T* __restrict__ vy,
+                                             T* __restrict__ vz, const T (&ox)[G], const T (&oy)[G], const T (&oz)[G]) {
+    if (VEC && i + G <= n) {
+        store_group(vx + i, ox);
+        store_group(vy + i, oy);
+        store_group(vz + i, oz);
+    } else {
+#pragma unroll
+        for (int e = 0; e < G; ++e) {
+            if (i + e < n) {
+                vx[i + e] = ox[e];
+                vy[i + e] = oy[e];
+                vz[i + e] = oz[e];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- kappagen_sample
+template <typename T, bool VEC>
+__global__ void __launch_bounds__(kThreads)
+sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
+              T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    constexpr int G = 16 / sizeof(T);
+    constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+#pragma unroll
+        for (int j = 0; j < kGroups; ++j) {
+            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+            if (i < n) {
+                T ox[G], oy[G], oz[G];
+#pragma unroll
+                for (int e = 0; e < G; ++e) {
+                    uint32_t w0, w1, w2;
+                    particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
+                    velocity(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                }
+                store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- kappagen_sample_cells
+// Pre-kernel: Table I lines 1-4 per cell, in double, into the workspace (one Coef<T> per cell).
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict__ theta, Coef<T>* __restrict__ W) {
+    const int64_t cell = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (cell >= ncell) return;
+    const double kap = (double)kappa[cell], th = (double)theta[cell];
+    const bool ok = isfinite(kap) && isfinite(th) && kap > 1.5 && th >= 0.0;
+    const double ks = ok ? kap - 0.5 : 1.0;
+    const double lnB = lgamma(1.5) + lgamma(ks) - lgamma(ks + 1.5);   // ln B(3/2, kappa*)
+    const TableIParams<double> P = table1_params<double>(ok ? kap : 2.5, lnB, c_approx_f64(ok ? kap : 2.5));
+    Coef<T> C = make_coef<T, double>(P, th);
+    if (!ok) C.theta = (T)nan("");                                    // whole cell becomes NaN
+    W[cell] = C;
+}
+
+template <typename T, bool VEC>
+__global__ void __launch_bounds__(kThreads)
+sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t offset, const __grid_constant__ PhiloxKeys K,
+                    const Coef<T>* __restrict__ W, const T* __restrict__ drift, int64_t drift_stride,
+                    T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    constexpr int G = 16 / sizeof(T);
+    constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+#pragma unroll
+        for (int j = 0; j < kGroups; ++j) {
+            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+            if (i < n) {
+                const int64_t cell0 = i / (int64_t)ppc;
+                const uint32_t rem = (uint32_t)(i - cell0 * (int64_t)ppc);
+                T ox[G], oy[G], oz[G];
+#pragma unroll
+                for (int e = 0; e < G; ++e) {
+                    int64_t cell = cell0 + (int64_t)((rem + (uint32_t)e) / ppc);
+                    if (i + e >= n) cell = cell0;                     // lanes past the end: stay in bounds
+                    const Coef<T> C = W[cell];
+                    uint32_t w0, w1, w2;
+                    particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
+                    velocity(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                    if (drift != nullptr) {
+                        const T* d = drift + 3 * cell * drift_stride;
+                        ox[e] += d[0];
+                        oy[e] += d[1];
+                        oz[e] += d[2];
+                    }
+                }
+                store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- test hooks
+__global__ void __launch_bounds__(kThreads)
+words_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,
+             uint32_t* __restrict__ o1, uint32_t* __restrict__ o2) {
+    for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
+        uint32_t w0, w1, w2;
+        particle_words(offset + (uint64_t)i, K, w0, w1, w2);
+        o0[i] = w0;
+        o1[i] = w1;
+        o2[i] = w2;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+velocity_of_words_kernel(int64_t n, const uint32_t* __restrict__ w0, const uint32_t* __restrict__ w1,
+                         const uint32_t* __restrict__ w2, const __grid_constant__ Coef<T> C,
+                         T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
+        T x, y, z;
+        velocity(w0[i], w1[i], w2[i], C, x, y, z);
+        vx[i] = x;
+        vy[i] = y;
+        vz[i] = z;
+    }
+}
+
+}  // namespace kappagen

@@ -1,0 +1,68 @@
+// philox.cuh -- register-resident Philox4x32-10 for the kappagen kernels (step S1 of DESIGN.md).
+//
+// The RNG is fixed by BASELINE.json's north_star (the paper says only "generate U1,U2,U3 ~
+// Uniform(0,1)", Table I line 5).  Algorithm: Salmon, Moraes, Dror, Shaw, "Parallel
+// random numbers: as easy as 1, 2, 3" (SC'11).  Written from that description for this kernel; no
+// code is shared with oracle/.
+//
+// Layout (reading R6): particle g uses counter (lo32 g, hi32 g, c2, c3) and key
+// (lo32 seed, hi32 seed); the samplers use c2 = c3 = 0, the rejection baseline uses c2 = trial
+// number and c3 = stream id.  The ten round keys depend only on the seed, so the host expands them
+// once (PhiloxKeys) and they reach the kernel through the constant bank: the per-particle cost is
+// 10 rounds x (2 IMAD.WIDE + 2 LOP3), less what constant propagation removes when c2 = c3 = 0.
+#pragma once
+#include <cstdint>
+
+namespace kappagen {
+
+struct PhiloxKeys {
+    uint32_t k0[10];
+    uint32_t k1[10];
+};
+
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;  // multiplies counter word 0
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;  // multiplies counter word 2
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;  // key schedule: golden ratio
+constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;  // key schedule: sqrt(3) - 1
+
+inline PhiloxKeys philox_expand_keys(uint64_t seed) {
+    PhiloxKeys K;
+    uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        K.k0[r] = a;
+        K.k1[r] = b;
+        a += kPhiloxW0;
+        b += kPhiloxW1;
+    }
+    return K;
+}
+
+#ifdef __CUDACC__
+// One Philox4x32-10 block.  w3 is computed only if the caller uses it (dead code otherwise).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const PhiloxKeys& K, uint32_t& w0, uint32_t& w1,
+                                              uint32_t& w2, uint32_t& w3) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0;  // IMAD.WIDE.U32
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];  // LOP3
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    w0 = c0; w1 = c1; w2 = c2; w3 = c3;
+}
+
+// The three words particle g consumes (w3 is drawn and discarded, reading R4).
+__device__ __forceinline__ void particle_words(uint64_t g, const PhiloxKeys& K, uint32_t& w0,
+                                               uint32_t& w1, uint32_t& w2) {
+    uint32_t w3;
+    philox4x32_10((uint32_t)g, (uint32_t)(g >> 32), 0u, 0u, K, w0, w1, w2, w3);
+    (void)w3;
+}
+#endif  // __CUDACC__
+
+}  // namespace kappagen

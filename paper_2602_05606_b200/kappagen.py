@@ -1,0 +1,188 @@
+"""Thin ctypes binding over libkappagen (include/kappagen.h).  Argument marshalling only: every step
+of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used to allocate device
+memory and to name the current stream; tensors are passed as raw pointers.
+
+There is no CPU fallback.  If libkappagen.so has not been built, the first call raises
+KappagenNotBuilt with the build command; on a machine without a CUDA device the library returns
+KAPPAGEN_ECUDA and the binding raises KappagenError.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+F32, F64 = 0, 1
+OK, EINVAL, ENULL, EALIGN, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4, -5
+_STATUS = {EINVAL: "KAPPAGEN_EINVAL", ENULL: "KAPPAGEN_ENULL", EALIGN: "KAPPAGEN_EALIGN",
+           EWORKSPACE: "KAPPAGEN_EWORKSPACE", ECUDA: "KAPPAGEN_ECUDA"}
+_SO = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libkappagen.so")
+_lib = None
+
+
+class KappagenNotBuilt(RuntimeError):
+    pass
+
+
+class KappagenError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__("%s (%d): %s" % (_STATUS.get(status, "?"), status, text))
+        self.status = status
+
+
+def lib() -> ctypes.CDLL:
+    """Load libkappagen.so (in-tree).  Fails loudly when it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise KappagenNotBuilt("%s is missing: build it with `python -m paper_2602_05606_b200.build` "
+                                   "(or __graft_entry__.build()); there is no CPU fallback" % _SO)
+        L = ctypes.CDLL(_SO)
+        i64, u64, f64, i32, vp, sz = (ctypes.c_int64, ctypes.c_uint64, ctypes.c_double, ctypes.c_int32,
+                                      ctypes.c_void_p, ctypes.c_size_t)
+        ci = ctypes.c_int
+        L.kappagen_sample.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp]
+        L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
+        L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
+        L.kappagen_cells_workspace_bytes.restype = sz
+        L.kappagen_sample_host.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp]
+        L.kappagen_baseline_mt.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp, vp]
+        L.kappagen_words.argtypes = [i64, u64, u64, vp, vp, vp, vp]
+        L.kappagen_velocity_of_words.argtypes = [i64, vp, vp, vp, f64, f64, ci, vp, vp, vp, vp]
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
+        L.kappagen_last_error.restype = ctypes.c_char_p
+        for name in ("kappagen_sample", "kappagen_sample_cells", "kappagen_sample_host", "kappagen_baseline_mt",
+                     "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version"):
+            getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    return lib().kappagen_last_error().decode()
+
+
+def version() -> int:
+    return lib().kappagen_version()
+
+
+def _check(rc: int) -> None:
+    if rc != OK:
+        raise KappagenError(rc, last_error())
+
+
+def _dtype_code(dtype) -> int:
+    if dtype in (torch.float32, "f32", F32):
+        return F32
+    if dtype in (torch.float64, "f64", F64):
+        return F64
+    raise ValueError("dtype must be float32/'f32' or float64/'f64'")
+
+
+def _torch_dtype(code: int):
+    return torch.float32 if code == F32 else torch.float64
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        if not torch.cuda.is_available():
+            return 0        # host-side argument checks still work; anything that launches returns KAPPAGEN_ECUDA
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _planes(n: int, code: int, out, device):
+    if out is None:
+        return tuple(torch.empty(n, dtype=_torch_dtype(code), device=device) for _ in range(3))
+    vx, vy, vz = out
+    for t in (vx, vy, vz):
+        if t.dtype != _torch_dtype(code) or t.numel() < n or not t.is_contiguous():
+            raise ValueError("output planes must be contiguous, of the requested dtype, with >= n elements")
+    return vx, vy, vz
+
+
+def params(kappa: float):
+    """Table I lines 1-4 on the host: (kappa*, a, b, c)."""
+    v = [ctypes.c_double() for _ in range(4)]
+    _check(lib().kappagen_params(kappa, *[ctypes.byref(x) for x in v]))
+    return tuple(x.value for x in v)
+
+
+def sample(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", out=None,
+           stream=None, device="cuda"):
+    """kappagen_sample: returns (vx, vy, vz) device tensors (or fills `out`)."""
+    code = _dtype_code(dtype)
+    vx, vy, vz = _planes(n, code, out, device)
+    _check(lib().kappagen_sample(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
+                                 _stream(stream)))
+    return vx, vy, vz
+
+
+def cells_workspace_bytes(ncell: int, dtype="f32") -> int:
+    return lib().kappagen_cells_workspace_bytes(ncell, _dtype_code(dtype))
+
+
+def sample_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0,
+                 seed: int = 0, offset: int = 0, out=None, workspace=None, stream=None):
+    """kappagen_sample_cells: kappa, theta (and drift) are device tensors of the output dtype."""
+    code = _dtype_code(kappa.dtype)
+    ncell = kappa.numel()
+    if theta.dtype != kappa.dtype or theta.numel() != ncell or (drift is not None and drift.dtype != kappa.dtype):
+        raise ValueError("kappa, theta and drift must share dtype; kappa and theta must share length")
+    vx, vy, vz = _planes(ncell * ppc, code, out, kappa.device)
+    need = cells_workspace_bytes(ncell, code)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    _check(lib().kappagen_sample_cells(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
+                                       drift.data_ptr() if drift is not None else None, drift_stride, seed, offset,
+                                       code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), workspace.data_ptr(),
+                                       workspace.numel() * workspace.element_size(), _stream(stream)))
+    return vx, vy, vz
+
+
+def sample_host(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", out=None,
+                pin: bool = True):
+    """kappagen_sample_host: host (CPU) tensors in, filled synchronously; the end-to-end path."""
+    code = _dtype_code(dtype)
+    if out is None:
+        out = tuple(torch.empty(n, dtype=_torch_dtype(code), pin_memory=pin) for _ in range(3))
+    vx, vy, vz = out
+    for t in (vx, vy, vz):
+        if t.is_cuda or t.dtype != _torch_dtype(code) or t.numel() < n or not t.is_contiguous():
+            raise ValueError("sample_host needs contiguous CPU tensors of the requested dtype")
+    _check(lib().kappagen_sample_host(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr()))
+    return vx, vy, vz
+
+
+def baseline_mt(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", out=None,
+                trip_counters=None, stream=None, device="cuda"):
+    """kappagen_baseline_mt: the rejection-based comparison generator (exact Kappa distribution)."""
+    code = _dtype_code(dtype)
+    vx, vy, vz = _planes(n, code, out, device)
+    if trip_counters is not None and (trip_counters.dtype not in (torch.int64, torch.uint64) or trip_counters.numel() < 2):
+        raise ValueError("trip_counters must be a device tensor of two 64-bit integers")
+    _check(lib().kappagen_baseline_mt(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
+                                      _stream(stream), trip_counters.data_ptr() if trip_counters is not None else None))
+    return vx, vy, vz
+
+
+def words(n: int, seed: int, offset: int = 0, stream=None, device="cuda"):
+    """kappagen_words: the Philox words particle i consumes, as three int32 tensors holding uint32 bits."""
+    w = tuple(torch.empty(n, dtype=torch.int32, device=device) for _ in range(3))
+    _check(lib().kappagen_words(n, seed, offset, w[0].data_ptr(), w[1].data_ptr(), w[2].data_ptr(), _stream(stream)))
+    return w
+
+
+def velocity_of_words(w0, w1, w2, kappa: float, theta: float, dtype="f32", stream=None):
+    """kappagen_velocity_of_words: S2-S6 on caller-chosen words (int32 device tensors holding uint32 bits)."""
+    code = _dtype_code(dtype)
+    n = w0.numel()
+    for w in (w0, w1, w2):
+        if w.dtype != torch.int32 or w.numel() != n or not w.is_contiguous():
+            raise ValueError("words must be contiguous int32 tensors of equal length")
+    vx, vy, vz = _planes(n, code, None, w0.device)
+    _check(lib().kappagen_velocity_of_words(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(), kappa, theta, code,
+                                            vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
+    return vx, vy, vz

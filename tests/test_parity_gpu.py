@@ -1,0 +1,171 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeds and offsets.  Words bit-exact; velocities within 1e-12 (fp64) / 4e-6 (fp32) strict
+per-component relative error (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from gpu_util import TAIL_BITS, TOL, max_rel_err, rel_err, report, u32
+from paper_2602_05606_b200 import kappagen as kg
+from paper_2602_05606_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+KAPPAS = wl.C2_KAPPAS
+
+
+def ref_sample(n, kappa, theta, seed, offset=0):
+    return oracle.sample(n, kappa, theta, seed, offset)
+
+
+# ------------------------------------------------------------------ S1: words, bit-exact
+@pytest.mark.parametrize("seed,offset,n", [(0, 0, 1_000_000), (1, 0, 4097), (42, 2**32 - 1000, 2000),
+                                           (123, 3 * 2**28 - 5, 4101), (0xA4093822_299F31D0, 2**40 + 7, 1000),
+                                           (7, 2**64 - 500, 1000)])
+def test_words_bit_exact(seed, offset, n):
+    got = kg.words(n, seed, offset)
+    want = oracle.words(n, seed, offset % 2**64)
+    for g, w in zip(got, want):
+        assert np.array_equal(u32(g), w)
+
+
+# ------------------------------------------------------------------ config 1: full element-wise parity, fp64
+def test_config1_fp64_full_parity():
+    c = wl.C1
+    got = kg.sample(c.n, c.kappa, c.theta, c.seed, c.offset, "f64")
+    want = ref_sample(c.n, c.kappa, c.theta, c.seed, c.offset)
+    err = max_rel_err(got, want)
+    report(test="config1_fp64", max_rel_err=err)
+    assert err <= TOL["f64"], err
+
+
+@pytest.mark.parametrize("kappa", KAPPAS)
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_sample_parity_1e6_per_kappa(kappa, dtype):
+    n, theta, seed = 1_000_003, 1.0, 1               # ragged: not a multiple of the tile or of the vector width
+    got = kg.sample(n, kappa, theta, seed, 0, dtype)
+    want = ref_sample(n, kappa, theta, seed, 0)
+    err = max_rel_err(got, want)
+    report(test="sample_1e6", kappa=kappa, dtype=dtype, max_rel_err=err)
+    assert err <= TOL[dtype], err
+
+
+# ------------------------------------------------------------------ S2-S6 on chosen words: both ends of every uniform
+@pytest.mark.parametrize("kappa", KAPPAS + (15.0,))
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_edge_words_whole_range(kappa, dtype):
+    w = wl.edge_words(n_random=20000)
+    rng = np.random.Generator(np.random.PCG64(5))
+    w0 = np.concatenate([w, rng.permutation(w), w])
+    w1 = np.concatenate([rng.permutation(w), w, w])
+    w2 = np.concatenate([rng.permutation(w), rng.permutation(w), w])
+    theta = 0.37
+    dev = [torch.from_numpy(a.view(np.int32)).cuda() for a in (w0, w1, w2)]
+    got = kg.velocity_of_words(*dev, kappa, theta, dtype)
+    want = oracle.velocity_of_words(w0, w1, w2, kappa, theta)
+    errs = np.maximum.reduce([rel_err(g.cpu().numpy(), r) for g, r in zip(got, want)])
+    tail = (w0 >= 2**32 - 2**TAIL_BITS) | (w0 < 2**TAIL_BITS)
+    bulk_err, tail_err = float(errs[~tail].max()), float(errs[tail].max())
+    report(test="edge_words", kappa=kappa, dtype=dtype, bulk_max_rel_err=bulk_err, tail_max_rel_err=tail_err,
+           n_tail=int(tail.sum()))
+    assert bulk_err <= TOL[dtype], bulk_err
+    # the tail region u -> 1 (and the head u -> 0) is reported separately; this implementation holds
+    # the same tolerance there, so gate it too
+    assert tail_err <= TOL[dtype], tail_err
+
+
+# ------------------------------------------------------------------ ragged sizes, misaligned planes, streams
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_ragged_sizes_and_misaligned_planes(dtype):
+    kappa, theta, seed, off = 3.0, 1.0, 9, 12345
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    full = kg.sample(9001, kappa, theta, seed, off, dtype)
+    for n in (0, 1, 3, 5, 127, 4097, 9001):
+        got = kg.sample(n, kappa, theta, seed, off, dtype)
+        for g, f in zip(got, full):
+            assert torch.equal(g, f[:n])
+        # planes offset by one element: not 16-byte aligned -> scalar-store path, same values
+        buf = [torch.full((n + 8,), float("nan"), dtype=tdt, device="cuda") for _ in range(3)]
+        out = tuple(b[1:] for b in buf)
+        kg.sample(n, kappa, theta, seed, off, dtype, out=out)
+        for b, f in zip(buf, full):
+            assert torch.equal(b[1:n + 1], f[:n])
+            assert torch.isnan(b[0]) and torch.isnan(b[n + 1:]).all()     # nothing written out of range
+
+
+def test_two_streams_concurrently():
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    n = 1 << 20
+    with torch.cuda.stream(s1):
+        a = kg.sample(n, 2.0, 1.0, 5, 0, "f32", stream=s1)
+    with torch.cuda.stream(s2):
+        b = kg.sample(n, 2.0, 1.0, 5, n, "f32", stream=s2)
+    torch.cuda.synchronize()
+    whole = kg.sample(2 * n, 2.0, 1.0, 5, 0, "f32")
+    torch.cuda.synchronize()
+    for x, y, w in zip(a, b, whole):
+        assert torch.equal(torch.cat([x, y]), w)
+
+
+def test_theta_zero_and_status_codes():
+    vx, vy, vz = kg.sample(1000, 2.5, 0.0, 1, 0, "f32")
+    assert (vx == 0).all() and (vy == 0).all() and (vz == 0).all()
+    with pytest.raises(kg.KappagenError) as e:
+        kg.sample(10, 1.5, 1.0, 0)
+    assert e.value.status == kg.EINVAL
+    buf = torch.empty(64, dtype=torch.uint8, device="cuda")
+    rc = kg.lib().kappagen_sample(4, 2.0, 1.0, 0, 0, kg.F64, buf.data_ptr() + 4, buf.data_ptr() + 8, buf.data_ptr() + 16, None)
+    assert rc == kg.EALIGN
+
+
+# ------------------------------------------------------------------ chunk continuation (config 5, small and full)
+def test_chunked_equals_one_shot_small():
+    n, chunks = 300_007, 3
+    one = kg.sample(n, 1.6, 1.0, 123, 10, "f32")
+    parts = [torch.empty(n, dtype=torch.float32, device="cuda") for _ in range(3)]
+    for j in range(chunks):
+        b, e = wl.shard_range(n, j, chunks)
+        kg.sample(e - b, 1.6, 1.0, 123, 10 + b, "f32", out=tuple(p[b:e] for p in parts))
+    for p, o in zip(parts, one):
+        assert torch.equal(p, o)
+
+
+def test_config5_chunked_2pow30_bit_identical_and_sampled_parity():
+    c = wl.C5
+    n, chunk = c.n, c.n // wl.C5_CHUNKS
+    one = kg.sample(n, c.kappa, c.theta, c.seed, 0, "f32")
+    parts = tuple(torch.empty(n, dtype=torch.float32, device="cuda") for _ in range(3))
+    for j in range(wl.C5_CHUNKS):
+        kg.sample(chunk, c.kappa, c.theta, c.seed, j * chunk, "f32", out=tuple(p[j * chunk:(j + 1) * chunk] for p in parts))
+    torch.cuda.synchronize()
+    for p, o in zip(parts, one):
+        assert torch.equal(p, o)
+    del parts
+    worst = 0.0
+    blocks = [0, n - 4096] + [j * chunk - 2048 for j in range(1, wl.C5_CHUNKS)] + [int(k) * 4096 for k in
+              np.random.Generator(np.random.PCG64(1)).integers(0, n // 4096, size=40)]
+    for b in blocks:
+        want = ref_sample(4096, c.kappa, c.theta, c.seed, b)
+        worst = max(worst, max_rel_err([o[b:b + 4096] for o in one], want))
+    report(test="config5_sampled", max_rel_err=worst, heavy_tail_vmax=float(max(o.abs().max().item() for o in one)))
+    assert worst <= TOL["f32"], worst
+
+
+# ------------------------------------------------------------------ config 3 at full size, sampled
+@pytest.mark.parametrize("cfg", [wl.C3_F32, wl.C3_F64], ids=lambda c: c.name)
+def test_config3_full_size_sampled_parity(cfg):
+    got = kg.sample(cfg.n, cfg.kappa, cfg.theta, cfg.seed, cfg.offset, cfg.dtype)
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.PCG64(3))
+    blocks = [0, cfg.n - 4096] + [int(k) * 4096 for k in rng.integers(0, cfg.n // 4096, size=60)]
+    worst = 0.0
+    for b in blocks:
+        want = ref_sample(4096, cfg.kappa, cfg.theta, cfg.seed, cfg.offset + b)
+        worst = max(worst, max_rel_err([g[b:b + 4096] for g in got], want))
+    report(test="config3_sampled", dtype=cfg.dtype, max_rel_err=worst)
+    assert worst <= TOL[cfg.dtype], worst
+    # properties that hold at any size: no NaN/inf anywhere, speed bounded by the largest 32-bit word's
+    sp2 = got[0].double() ** 2 + got[1].double() ** 2 + got[2].double() ** 2
+    xmax = oracle.x_of_w0([2**32 - 1], cfg.kappa)[0] * cfg.theta**2
+    assert torch.isfinite(sp2).all() and sp2.max().item() <= xmax * (1 + 1e-5) and sp2.min().item() > 0
