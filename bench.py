@@ -1,0 +1,284 @@
+"""bench.py -- throughput of the kappagen hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f32|f64] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (S1-S6: Philox -> q-exponential inverse -> direction ->
+SoA stores) over one batch: kappagen_sample(2^28, kappa=2.0, theta=0.1, seed=42, offset=step*2^28)
+= BASELINE.json configs[2], the configuration its metric ("particles/s ... at 2^28 particles") is
+quoted on.  Under torchrun every rank does the same amount of work on its own index range (weak
+scaling, no collective: SURVEY.md section 8(e)).  Prints ONE JSON line on rank 0.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands, one thread) on a bounded sample of
+the same workload; it is a deliberately slow checker, not a competitor.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "kappa_particles_per_second"
+UNIT = "particles/s"
+N_STEP = 1 << 28                       # particles per step per GPU (configs[2])
+KAPPA, THETA, SEED = 2.0, 0.1, 42
+REF_SAMPLE = 1 << 20                   # particles per step of the --impl reference arm
+CPU_BASELINE_SAMPLE = 1 << 24          # particles of the cpu_baseline leg (~10-20 s of one core)
+FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum of one sample_kernel launch at 2^28 particles, from the
+# ncu --set full capture summarised in profiles/ (None until a capture exists for that dtype).
+NCU_TRAFFIC_BYTES = {"f32": None, "f64": None}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--dtype", choices=["f32", "f64"], default="f32")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / baseline / cells extra timings")
+    return ap.parse_args()
+
+
+def config_dict(dtype, world):
+    return {"workload": "BASELINE.json configs[2]: 2^28 particles per step per GPU, kappa=2.0, theta=0.1, seed=42, "
+                        "%s SoA vx/vy/vz, Philox offset advances by 2^28 per step" % dtype,
+            "particles_per_step_per_gpu": N_STEP, "kappa": KAPPA, "theta": THETA, "seed": SEED,
+            "parallelism": "index-range sharding x%d, no collective" % world,
+            "l2": "write-only path; each step writes %.2f GB of output (> 126 MB L2), no L2 flush needed"
+                  % (N_STEP * 3 * (4 if dtype == "f32" else 8) / 1e9)}
+
+
+# --------------------------------------------------------------------------- reference arm (CPU oracle)
+def oracle_rate(n, offset=0):
+    """Time oracle.sample on n particles of the workload, one thread.  Returns particles/s."""
+    import oracle
+    t0 = time.perf_counter()
+    oracle.sample(n, KAPPA, THETA, SEED, offset)
+    return n / (time.perf_counter() - t0)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.lib()
+    for w in range(max(args.warmup, 0)):
+        oracle.sample(REF_SAMPLE, KAPPA, THETA, SEED, w * REF_SAMPLE)
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        oracle.sample(REF_SAMPLE, KAPPA, THETA, SEED, s * REF_SAMPLE)
+    dt = time.perf_counter() - t0
+    value = args.steps * REF_SAMPLE / dt
+    sample = "%d particles per step of configs[2] (kappa=2.0, theta=0.1, seed=42), long double, 1 thread" % REF_SAMPLE
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(args.dtype, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake_slowdown"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# --------------------------------------------------------------------------- our arm
+def time_launches(fn, steps, warmup, torch):
+    """Run fn(step) warmup+steps times on the current stream; returns (total_ms, [per-launch ms])."""
+    for s in range(warmup):
+        fn(s)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_begin.record()
+    for s in range(steps):
+        ev[s][0].record()
+        fn(warmup + s)
+        ev[s][1].record()
+    t_end.record()
+    torch.cuda.synchronize()
+    return t_begin.elapsed_time(t_end), [a.elapsed_time(b) for a, b in ev]
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_05606_b200 import kappagen as kg
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    kg.lib()                                            # fail loudly now if libkappagen.so is missing
+    dtype, n = args.dtype, N_STEP
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    es = 4 if dtype == "f32" else 8
+    planes = tuple(torch.empty(n, dtype=tdt, device="cuda") for _ in range(3))
+    stream = torch.cuda.current_stream()
+
+    def step(s):
+        # rank r owns the index range [ (s*world + r) * n, +n ): contiguous shards, no exchange
+        kg.sample(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, out=planes, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for s in range(max(args.warmup, 3)):
+        step(s)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    total_ms, per_launch = time_launches(step, args.steps, 0, torch)
+    barrier()
+    clocks = sampler.stop()
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = world * n * args.steps / (total_ms * 1e-3)
+    kern_ms = sum(per_launch) / len(per_launch)
+
+    # ---- end to end through the C ABI with HOST buffers (device->host copies inside the timed region)
+    host = tuple(torch.empty(n, dtype=tdt, pin_memory=True) for _ in range(3))
+    kg.sample_host(n, KAPPA, THETA, SEED, rank * n, dtype, out=host)            # warm-up (also faults the pages in)
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(args.e2e_steps):
+        kg.sample_host(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, out=host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * n * args.e2e_steps / float(te.item())
+    checksum = float(host[0][:1024].double().abs().sum())                         # the host result is read
+    del host
+
+    line = None
+    if rank == 0:
+        peak, which = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                peak, which = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+        except Exception:
+            pass
+        achieved = 3 * es * n / (kern_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": dtype, "data": "synthetic", "config": config_dict(dtype, world),
+            "clocks": clocks, "gpu_launches": args.steps,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 3 * es * n * world,
+                    "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES[dtype], "peak_source": which, "kernel": "sample_kernel<%s,true>" % dtype,
+                         "algorithmic_bytes_per_launch": 3 * es * n, "kernel_ms": kern_ms,
+                         "kernel_ms_min": min(per_launch), "kernel_ms_max": max(per_launch)},
+        }
+        if world == 1 and not args.no_extras:
+            line["extras"] = extras(kg, torch, dtype)
+        if world == 1:
+            rate = oracle_rate(CPU_BASELINE_SAMPLE)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "first %d particles of configs[2] (kappa=2.0, theta=0.1, seed=42), "
+                                              "oracle.sample in long double on one host thread" % CPU_BASELINE_SAMPLE}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def extras(kg, torch, dtype):
+    """Reported beside the headline (N=1 only): the other dtype and the rejection baseline at the same size."""
+    out = {}
+    n = N_STEP
+    st = torch.cuda.current_stream()
+    p64 = tuple(torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    p32 = tuple(x.view(torch.float32)[:n] for x in p64)
+    planes = {"f32": p32, "f64": p64}
+    other = "f64" if dtype == "f32" else "f32"
+    es = {"f32": 4, "f64": 8}
+    _, ms = time_launches(lambda s: kg.sample(n, KAPPA, THETA, SEED, s * n, other, out=planes[other], stream=st), 10, 3, torch)
+    k = sum(ms) / len(ms)
+    out["sample_" + other] = {"particles_per_s": n / (k * 1e-3), "kernel_ms": k, "write_GBps": 3 * es[other] * n / (k * 1e-3) / 1e9}
+    for dt in ("f32", "f64"):
+        _, ms = time_launches(lambda s: kg.baseline_mt(n, KAPPA, THETA, SEED, s * n, dt, out=planes[dt], stream=st), 5, 2, torch)
+        k = sum(ms) / len(ms)
+        out["baseline_mt_" + dt] = {"particles_per_s": n / (k * 1e-3), "kernel_ms": k, "write_GBps": 3 * es[dt] * n / (k * 1e-3) / 1e9}
+    return out
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
