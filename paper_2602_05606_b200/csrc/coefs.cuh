@@ -19,18 +19,37 @@ struct TableIParams {
     F kstar, a, b, c;
 };
 
-// Per-(kappa, theta) constants in the kernel's arithmetic type.  32 bytes (float) / 64 bytes
-// (double): the cells path stores one of these per cell in the workspace.
-template <typename T>
-struct alignas(16) Coef {
-    T s;      // 1/kappa*
-    T a;      // Eq. (13)
-    T ck;     // c kappa*
-    T bk4;    // 4 b kappa*
-    T k2;     // 2 kappa*
-    T i2b;    // 1/(2b)
-    T theta;  // most probable speed; NaN marks an invalid cell
-    T pad;
+// Per-(kappa, theta) constants in the kernel's arithmetic type: 64 bytes (double), 32 bytes (float);
+// the cells path stores one per cell in the workspace.
+template <typename T> struct Coef;
+
+template <>
+struct alignas(16) Coef<double> {
+    double s;      // 1/kappa*
+    double a;      // Eq. (13)
+    double ck;     // c kappa*
+    double bk4;    // 4 b kappa*
+    double k2;     // 2 kappa*
+    double i2b;    // 1/(2b)
+    double theta;  // most probable speed; NaN marks an invalid cell
+    double pad;
+};
+
+// The float chain returns 2V = sqrt(num/den) with
+//   A >= 0: num = k2 Y, den = T;   A < 0: num = th4 T, den = b2;   T = |A| + sqrt(A^2 + bk4 Y).
+// Folded (uniform parameters, theta in [2^-30, 2^30]): k2 = 8 kappa* theta^2, th4 = 4 theta^2, theta = 1,
+// so the speed needs no further multiply.  Unfolded (per-cell parameters, theta = 0 or extreme):
+// k2 = 8 kappa*, th4 = 4, and the kernel multiplies by theta (NaN marks an invalid cell).
+template <>
+struct alignas(16) Coef<float> {
+    float s;      // 1/kappa*
+    float a;      // Eq. (13)
+    float ck;     // c kappa*
+    float bk4;    // 4 b kappa*
+    float k2;     // 8 kappa* [theta^2]
+    float b2;     // 2 b
+    float th4;    // 4 [theta^2]
+    float theta;  // theta, or 1 when folded
 };
 
 #ifdef __CUDACC__
@@ -73,18 +92,36 @@ KAPPAGEN_HD inline TableIParams<F> table1_params(F kappa, F lnB, F c) {
     return P;
 }
 
-template <typename T, typename F>
-KAPPAGEN_HD inline Coef<T> make_coef(const TableIParams<F>& P, F theta) {
-    Coef<T> C;
-    C.s = (T)(F(1.0) / P.kstar);
-    C.a = (T)P.a;
-    C.ck = (T)(P.c * P.kstar);
-    C.bk4 = (T)(F(4.0) * P.b * P.kstar);
-    C.k2 = (T)(F(2.0) * P.kstar);
-    C.i2b = (T)(F(1.0) / (F(2.0) * P.b));
-    C.theta = (T)theta;
-    C.pad = (T)0;
+template <typename F>
+KAPPAGEN_HD inline Coef<double> make_coef_f64(const TableIParams<F>& P, F theta) {
+    Coef<double> C;
+    C.s = (double)(F(1.0) / P.kstar);
+    C.a = (double)P.a;
+    C.ck = (double)(P.c * P.kstar);
+    C.bk4 = (double)(F(4.0) * P.b * P.kstar);
+    C.k2 = (double)(F(2.0) * P.kstar);
+    C.i2b = (double)(F(1.0) / (F(2.0) * P.b));
+    C.theta = (double)theta;
+    C.pad = 0.0;
     return C;
 }
+
+// fold: put theta^2 into k2/th4 (only when 4 theta^2 and everything it multiplies stay normal floats).
+template <typename F>
+KAPPAGEN_HD inline Coef<float> make_coef_f32(const TableIParams<F>& P, F theta, bool fold) {
+    Coef<float> C;
+    const F t2 = fold ? theta * theta : F(1.0);
+    C.s = (float)(F(1.0) / P.kstar);
+    C.a = (float)P.a;
+    C.ck = (float)(P.c * P.kstar);
+    C.bk4 = (float)(F(4.0) * P.b * P.kstar);
+    C.k2 = (float)(F(8.0) * P.kstar * t2);
+    C.b2 = (float)(F(2.0) * P.b);
+    C.th4 = (float)(F(4.0) * t2);
+    C.theta = fold ? 1.0f : (float)theta;
+    return C;
+}
+
+KAPPAGEN_HD inline bool theta_folds(double theta) { return theta >= 0x1p-30 && theta <= 0x1p+30; }
 
 }  // namespace kappagen

@@ -40,12 +40,12 @@ TableIParams<double> host_table1(double kappa) {
     return D;
 }
 
-Coef<float> host_coef_f32(double kappa, double theta) {
-    return make_coef<float, long double>(table1_ld(kappa), (long double)theta);
+Coef<float> host_coef_f32(double kappa, double theta, bool fold) {
+    return make_coef_f32<long double>(table1_ld(kappa), (long double)theta, fold);
 }
 
 Coef<double> host_coef_f64(double kappa, double theta) {
-    return make_coef<double, long double>(table1_ld(kappa), (long double)theta);
+    return make_coef_f64<long double>(table1_ld(kappa), (long double)theta);
 }
 
 }  // namespace kappagen

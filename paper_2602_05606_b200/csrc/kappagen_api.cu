@@ -62,21 +62,32 @@ static int check_planes(const char* fn, int64_t n, int dtype, const void* vx, co
     return KAPPAGEN_OK;
 }
 
-template <typename T>
-static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, bool vec,
-                         T* vx, T* vy, T* vz, cudaStream_t st) {
+template <typename T, bool VEC, bool FOLD>
+static int launch_sample_as(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T* vx, T* vy, T* vz,
+                            cudaStream_t st) {
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
-    const int64_t tiles = (n + tile - 1) / tile;
     int grid = 0, rc;
-    if (vec) {
-        if ((rc = grid_for(sample_kernel<T, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_kernel<T, true><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
-    } else {
-        if ((rc = grid_for(sample_kernel<T, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_kernel<T, false><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
-    }
+    if ((rc = grid_for(sample_kernel<T, VEC, FOLD>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
+    sample_kernel<T, VEC, FOLD><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
+}
+
+static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec,
+                         float* vx, float* vy, float* vz, cudaStream_t st) {
+    const bool fold = theta_folds(theta);
+    const Coef<float> C = host_coef_f32(kappa, theta, fold);
+    if (vec) return fold ? launch_sample_as<float, true, true>(n, offset, K, C, vx, vy, vz, st)
+                         : launch_sample_as<float, true, false>(n, offset, K, C, vx, vy, vz, st);
+    return fold ? launch_sample_as<float, false, true>(n, offset, K, C, vx, vy, vz, st)
+                : launch_sample_as<float, false, false>(n, offset, K, C, vx, vy, vz, st);
+}
+
+static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec,
+                         double* vx, double* vy, double* vz, cudaStream_t st) {
+    const Coef<double> C = host_coef_f64(kappa, theta);
+    return vec ? launch_sample_as<double, true, false>(n, offset, K, C, vx, vy, vz, st)
+               : launch_sample_as<double, false, false>(n, offset, K, C, vx, vy, vz, st);
 }
 
 static int sample_on_stream(const char* fn, int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
@@ -90,9 +101,8 @@ static int sample_on_stream(const char* fn, int64_t n, double kappa, double thet
     }
     if (n == 0) return KAPPAGEN_OK;
     const PhiloxKeys K = philox_expand_keys(seed);
-    if (dtype == KAPPAGEN_F32)
-        return launch_sample<float>(n, offset, K, host_coef_f32(kappa, theta), vec, (float*)vx, (float*)vy, (float*)vz, st);
-    return launch_sample<double>(n, offset, K, host_coef_f64(kappa, theta), vec, (double*)vx, (double*)vy, (double*)vz, st);
+    if (dtype == KAPPAGEN_F32) return launch_sample(n, offset, K, kappa, theta, vec, (float*)vx, (float*)vy, (float*)vz, st);
+    return launch_sample(n, offset, K, kappa, theta, vec, (double*)vx, (double*)vy, (double*)vz, st);
 }
 
 template <typename T>
@@ -251,13 +261,19 @@ extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const u
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t tiles = (n + kThreads - 1) / kThreads;
     if (dtype == KAPPAGEN_F32) {
-        if ((rc = grid_for(velocity_of_words_kernel<float>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        velocity_of_words_kernel<float><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f32(kappa, theta),
-                                                                   (float*)vx, (float*)vy, (float*)vz);
+        const bool fold = theta_folds(theta);              // the same choice kappagen_sample makes
+        const Coef<float> C = host_coef_f32(kappa, theta, fold);
+        if (fold) {
+            if ((rc = grid_for(velocity_of_words_kernel<float, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            velocity_of_words_kernel<float, true><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, C, (float*)vx, (float*)vy, (float*)vz);
+        } else {
+            if ((rc = grid_for(velocity_of_words_kernel<float, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            velocity_of_words_kernel<float, false><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, C, (float*)vx, (float*)vy, (float*)vz);
+        }
     } else {
-        if ((rc = grid_for(velocity_of_words_kernel<double>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        velocity_of_words_kernel<double><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f64(kappa, theta),
-                                                                    (double*)vx, (double*)vy, (double*)vz);
+        if ((rc = grid_for(velocity_of_words_kernel<double, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        velocity_of_words_kernel<double, false><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f64(kappa, theta),
+                                                                           (double*)vx, (double*)vy, (double*)vz);
     }
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;

@@ -22,8 +22,11 @@ template <typename T> struct Vec128;
 template <> struct Vec128<float> { using type = float4; };
 template <> struct Vec128<double> { using type = double2; };
 
+// FOLD (float only): theta is folded into the coefficients, see coefs.cuh.
+template <bool FOLD>
 __device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<float>& C,
-                                         float& x, float& y, float& z) { velocity_f32(w0, w1, w2, C, x, y, z); }
+                                         float& x, float& y, float& z) { velocity_f32<FOLD>(w0, w1, w2, C, x, y, z); }
+template <bool FOLD>
 __device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<double>& C,
                                          double& x, double& y, double& z) { velocity_f64(w0, w1, w2, C, x, y, z); }
 
@@ -55,7 +58,7 @@ __device__ __forceinline__ void store_planes(int64_t i, int64_t n, T* __restrict
 }
 
 // ---------------------------------------------------------------- kappagen_sample
-template <typename T, bool VEC>
+template <typename T, bool VEC, bool FOLD>
 __global__ void __launch_bounds__(kThreads)
 sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
               T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
@@ -71,7 +74,7 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
                 for (int e = 0; e < G; ++e) {
                     uint32_t w0, w1, w2;
                     particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                    velocity(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                    velocity<FOLD>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
                 }
                 store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
             }
@@ -80,6 +83,14 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
 }
 
 // ---------------------------------------------------------------- kappagen_sample_cells
+template <typename T> __device__ __forceinline__ Coef<T> cell_coef(const TableIParams<double>& P, double theta);
+template <> __device__ __forceinline__ Coef<float> cell_coef<float>(const TableIParams<double>& P, double theta) {
+    return make_coef_f32<double>(P, theta, false);                     // per-cell theta: never folded
+}
+template <> __device__ __forceinline__ Coef<double> cell_coef<double>(const TableIParams<double>& P, double theta) {
+    return make_coef_f64<double>(P, theta);
+}
+
 // Pre-kernel: Table I lines 1-4 per cell, in double, into the workspace (one Coef<T> per cell).
 template <typename T>
 __global__ void __launch_bounds__(kThreads)
@@ -91,7 +102,7 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
     const double ks = ok ? kap - 0.5 : 1.0;
     const double lnB = lgamma(1.5) + lgamma(ks) - lgamma(ks + 1.5);   // ln B(3/2, kappa*)
     const TableIParams<double> P = table1_params<double>(ok ? kap : 2.5, lnB, c_approx_f64(ok ? kap : 2.5));
-    Coef<T> C = make_coef<T, double>(P, th);
+    Coef<T> C = cell_coef<T>(P, th);
     if (!ok) C.theta = (T)nan("");                                    // whole cell becomes NaN
     W[cell] = C;
 }
@@ -118,7 +129,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t offset, const __grid_const
                     const Coef<T> C = W[cell];
                     uint32_t w0, w1, w2;
                     particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                    velocity(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                    velocity<false>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
                     if (drift != nullptr) {
                         const T* d = drift + 3 * cell * drift_stride;
                         ox[e] += d[0];
@@ -145,14 +156,14 @@ words_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, u
     }
 }
 
-template <typename T>
+template <typename T, bool FOLD>
 __global__ void __launch_bounds__(kThreads)
 velocity_of_words_kernel(int64_t n, const uint32_t* __restrict__ w0, const uint32_t* __restrict__ w1,
                          const uint32_t* __restrict__ w2, const __grid_constant__ Coef<T> C,
                          T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
         T x, y, z;
-        velocity(w0[i], w1[i], w2[i], C, x, y, z);
+        velocity<FOLD>(w0[i], w1[i], w2[i], C, x, y, z);
         vx[i] = x;
         vy[i] = y;
         vz[i] = z;
