@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 #include "coefs.cuh"
 #include "math_f32.cuh"
+#include "math_f32x2.cuh"
 #include "math_f64.cuh"
 #include "philox.cuh"
 
@@ -29,6 +30,34 @@ __device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, 
 template <bool FOLD>
 __device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<double>& C,
                                          double& x, double& y, double& z) { velocity_f64(w0, w1, w2, C, x, y, z); }
+
+// One 128-bit group: G consecutive particles starting at global counter g0.  float: two packed pairs
+// (math_f32x2.cuh, bit-identical to the scalar chain); double: two scalar chains.
+template <bool FOLD>
+__device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<float>& C,
+                                                 float (&ox)[4], float (&oy)[4], float (&oz)[4]) {
+#pragma unroll
+    for (int e = 0; e < 4; e += 2) {
+        uint32_t w0[2], w1[2], w2[2];
+        particle_words(g0 + (uint64_t)e, K, w0[0], w1[0], w2[0]);
+        particle_words(g0 + (uint64_t)(e + 1), K, w0[1], w1[1], w2[1]);
+        float a[2], b[2], c[2];
+        velocity_pair_f32<FOLD>(w0, w1, w2, C, a, b, c);
+        ox[e] = a[0]; ox[e + 1] = a[1];
+        oy[e] = b[0]; oy[e + 1] = b[1];
+        oz[e] = c[0]; oz[e + 1] = c[1];
+    }
+}
+template <bool FOLD>
+__device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<double>& C,
+                                                 double (&ox)[2], double (&oy)[2], double (&oz)[2]) {
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        uint32_t w0, w1, w2;
+        particle_words(g0 + (uint64_t)e, K, w0, w1, w2);
+        velocity_f64(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+    }
+}
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
 __device__ __forceinline__ void store_group(float* p, const float (&v)[4]) {
@@ -70,12 +99,7 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
             const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
             if (i < n) {
                 T ox[G], oy[G], oz[G];
-#pragma unroll
-                for (int e = 0; e < G; ++e) {
-                    uint32_t w0, w1, w2;
-                    particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                    velocity<FOLD>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
-                }
+                group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox, oy, oz);
                 store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
             }
         }

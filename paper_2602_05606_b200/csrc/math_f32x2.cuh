@@ -1,0 +1,107 @@
+// math_f32x2.cuh -- the float chain of math_f32.cuh for TWO particles at a time on Blackwell's packed
+// fp32 instructions (PTX fma/mul/add.rn.f32x2 -> SASS FFMA2/FMUL2/FADD2, sm_100+).
+//
+// Why: the fp32 sampler is bound by instruction issue and by the FMA pipe (Philox's IMAD.WIDE alone holds
+// that pipe 4 cycles each); a packed instruction does two particles' FMA in one
+// issue slot.  MUFU, integer->float conversions and selects have no packed form and stay scalar on the two
+// halves of the register pair (no data movement: a f32x2 value IS two adjacent 32-bit registers).
+// Same arithmetic, same polynomials, same selects as math_f32.cuh -- results are bit-identical to it.
+#pragma once
+#include <cstdint>
+#include "coefs.cuh"
+#include "math_f32.cuh"
+
+namespace kappagen {
+
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f32x2 splat2(float c) { return pk2(c, c); }
+__device__ __forceinline__ void up2(f32x2 r, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(r)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+#define KG_MAP2(fn, v) ([&] { float a_, b_; up2((v), a_, b_); return pk2(fn(a_), fn(b_)); }())
+
+// 2V for two particles (see speed2_f32).
+__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, const Coef<float>& C) {
+    const f32x2 lg = KG_MAP2(mufu_lg2, add2(pk2((float)w0a, (float)w0b), splat2(0.5f)));
+    const f32x2 r = KG_MAP2(mufu_ex2, fma2(lg, splat2(0x1.555556p-2f), splat2(-0x1.555556p+3f)));
+    const f32x2 t1 = fma2(pk2((float)(uint32_t)(~w0a), (float)(uint32_t)(~w0b)), splat2(0x1p-32f), splat2(0x1p-33f));
+    const f32x2 p = mul2(r, r);
+    const f32x2 q1 = add2(r, splat2(1.0f));
+    const f32x2 S = mul2(mul2(t1, q1), KG_MAP2(mufu_rcp, add2(q1, p)));
+    f32x2 G = fma2(splat2(0x1.f5fc4cp-2f), p, splat2(0x1.a938e2p-3f));
+    G = fma2(G, p, splat2(0x1.7cda04p-2f));
+    G = fma2(G, p, splat2(0x1.ebbc5ap-2f));
+    G = fma2(G, p, splat2(0x1.715672p-1f));
+    G = fma2(G, p, splat2(0x1.715476p+0f));
+    const f32x2 m_small = mul2(mul2(p, splat2(C.s)), G);
+    const f32x2 m_large = mul2(KG_MAP2(mufu_lg2, S), splat2(-C.s));
+    float pa, pb, msa, msb, mla, mlb;
+    up2(p, pa, pb); up2(m_small, msa, msb); up2(m_large, mla, mlb);
+    const float ma = (pa < 0.25f) ? msa : mla, mb = (pb < 0.25f) ? msb : mlb;
+    const f32x2 m = pk2(ma, mb);
+    f32x2 R = fma2(splat2(0x1.93f00ep-10f), m, splat2(0x1.3823f8p-7f));
+    R = fma2(R, m, splat2(0x1.c6d326p-5f));
+    R = fma2(R, m, splat2(0x1.ebfb58p-3f));
+    R = fma2(R, m, splat2(0x1.62e430p-1f));
+    const f32x2 y_small = mul2(m, R);
+    const f32x2 y_large = add2(KG_MAP2(mufu_ex2, m), splat2(-1.0f));
+    float ysa, ysb, yla, ylb;
+    up2(y_small, ysa, ysb); up2(y_large, yla, ylb);
+    const f32x2 Y = pk2((ma < 0.5f) ? ysa : yla, (mb < 0.5f) ? ysb : ylb);
+    const f32x2 A = fma2(Y, splat2(-C.ck), splat2(C.a));
+    const f32x2 D = KG_MAP2(mufu_sqrt, fma2(A, A, mul2(Y, splat2(C.bk4))));
+    float Aa, Ab, Da, Db;
+    up2(A, Aa, Ab); up2(D, Da, Db);
+    const float Ta = fabsf(Aa) + Da, Tb = fabsf(Ab) + Db;
+    const f32x2 n_pos = mul2(Y, splat2(C.k2)), n_neg = mul2(pk2(Ta, Tb), splat2(C.th4));
+    float npa, npb, nna, nnb;
+    up2(n_pos, npa, npb); up2(n_neg, nna, nnb);
+    const bool posa = Aa >= 0.0f, posb = Ab >= 0.0f;
+    const f32x2 num = pk2(posa ? npa : nna, posb ? npb : nnb);
+    const f32x2 den = pk2(posa ? Ta : C.b2, posb ? Tb : C.b2);
+    return mul2(num, KG_MAP2(mufu_rsq, mul2(num, den)));
+}
+
+__device__ __forceinline__ void quadrant_f32(uint32_t w2, float sr, float cr, float& cphi, float& sphi) {
+    const uint32_t wq = w2 + 0x20000000u;
+    const bool odd = (wq & 0x40000000u) != 0u;
+    const float c0 = odd ? sr : cr;
+    const float s0 = odd ? cr : sr;
+    cphi = __uint_as_float(__float_as_uint(c0) ^ ((wq + 0x40000000u) & 0x80000000u));
+    sphi = __uint_as_float(__float_as_uint(s0) ^ (wq & 0x80000000u));
+}
+
+template <bool FOLD>
+__device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
+                                                  const Coef<float>& C, float (&vx)[2], float (&vy)[2], float (&vz)[2]) {
+    f32x2 V2 = speed2_f32x2(w0[0], w0[1], C);
+    if (!FOLD) V2 = mul2(V2, splat2(C.theta));
+    const f32x2 muh = fma2(pk2((float)(int32_t)(w1[0] ^ 0x80000000u), (float)(int32_t)(w1[1] ^ 0x80000000u)),
+                           splat2(0x1p-32f), splat2(0x1p-33f));
+    const f32x2 ef = pk2((float)min(w1[0], ~w1[0]), (float)min(w1[1], ~w1[1]));
+    const f32x2 e = fma2(ef, splat2(0x1p-32f), splat2(0x1p-33f));
+    const f32x2 ne = fma2(ef, splat2(-0x1p-32f), splat2(-0x1p-33f));
+    const f32x2 sth = KG_MAP2(mufu_sqrt, fma2(ne, e, e));
+    const f32x2 q = fma2(pk2((float)(int32_t)(w2[0] << 2), (float)(int32_t)(w2[1] << 2)), splat2(0x1p-32f), splat2(0x1p-31f));
+    const f32x2 z = mul2(q, q);
+    f32x2 sp = fma2(splat2(-0x1.2d9302p-8f), z, splat2(0x1.465e92p-4f));
+    sp = fma2(sp, z, splat2(-0x1.4abbbap-1f));
+    sp = fma2(sp, z, splat2(0x1.921fb6p+0f));
+    f32x2 cr = fma2(splat2(-0x1.4e35dap-6f), z, splat2(0x1.03ae64p-2f));
+    cr = fma2(cr, z, splat2(-0x1.3bd38cp+0f));
+    cr = fma2(cr, z, splat2(0x1.fffffep-1f));
+    const f32x2 sr = mul2(sp, q);
+    float sra, srb, cra, crb, ca, cb, sa, sb;
+    up2(sr, sra, srb); up2(cr, cra, crb);
+    quadrant_f32(w2[0], sra, cra, ca, sa);
+    quadrant_f32(w2[1], srb, crb, cb, sb);
+    const f32x2 Vs = mul2(V2, sth);
+    up2(mul2(V2, muh), vx[0], vx[1]);
+    up2(mul2(Vs, pk2(ca, cb)), vy[0], vy[1]);
+    up2(mul2(Vs, pk2(sa, sb)), vz[0], vz[1]);
+}
+
+}  // namespace kappagen
