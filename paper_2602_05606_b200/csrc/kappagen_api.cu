@@ -235,7 +235,7 @@ extern "C" int kappagen_words(int64_t n, uint64_t seed, uint64_t offset, uint32_
         return KAPPAGEN_EALIGN;
     }
     int grid = 0, rc;
-    if ((rc = grid_for(words_kernel, (n + kThreads - 1) / kThreads, &grid)) != KAPPAGEN_OK) return rc;
+    if ((rc = grid_for(words_kernel, (n + 4 * kThreads - 1) / (4 * kThreads), &grid)) != KAPPAGEN_OK) return rc;
     words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;

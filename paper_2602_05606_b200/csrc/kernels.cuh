@@ -31,18 +31,35 @@ template <bool FOLD>
 __device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<double>& C,
                                          double& x, double& y, double& z) { velocity_f64(w0, w1, w2, C, x, y, z); }
 
+// The Philox words of G consecutive particles starting at global counter g0.  Unless the low counter
+// word wraps inside the group (one group in 2^32 particles; a uniform branch everywhere else) the
+// particles share hi32(g) and with it the head of the Philox block (philox.cuh).
+template <int G>
+__device__ __forceinline__ void group_words(uint64_t g0, const PhiloxKeys& K, uint32_t (&w0)[G], uint32_t (&w1)[G],
+                                            uint32_t (&w2)[G]) {
+    const uint32_t lo = (uint32_t)g0, hi = (uint32_t)(g0 >> 32);
+    if (lo <= 0xFFFFFFFFu - (uint32_t)(G - 1)) {
+        const PhiloxHead H = philox_head(hi, K);
+#pragma unroll
+        for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < G; ++e) particle_words(g0 + (uint64_t)e, K, w0[e], w1[e], w2[e]);
+    }
+}
+
 // One 128-bit group: G consecutive particles starting at global counter g0.  float: two packed pairs
 // (math_f32x2.cuh, bit-identical to the scalar chain); double: two scalar chains.
 template <bool FOLD>
 __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<float>& C,
                                                  float (&ox)[4], float (&oy)[4], float (&oz)[4]) {
+    uint32_t w0[4], w1[4], w2[4];
+    group_words<4>(g0, K, w0, w1, w2);
 #pragma unroll
     for (int e = 0; e < 4; e += 2) {
-        uint32_t w0[2], w1[2], w2[2];
-        particle_words(g0 + (uint64_t)e, K, w0[0], w1[0], w2[0]);
-        particle_words(g0 + (uint64_t)(e + 1), K, w0[1], w1[1], w2[1]);
+        const uint32_t p0[2] = {w0[e], w0[e + 1]}, p1[2] = {w1[e], w1[e + 1]}, p2[2] = {w2[e], w2[e + 1]};
         float a[2], b[2], c[2];
-        velocity_pair_f32<FOLD>(w0, w1, w2, C, a, b, c);
+        velocity_pair_f32<FOLD>(p0, p1, p2, C, a, b, c);
         ox[e] = a[0]; ox[e + 1] = a[1];
         oy[e] = b[0]; oy[e + 1] = b[1];
         oz[e] = c[0]; oz[e + 1] = c[1];
@@ -51,12 +68,10 @@ __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& 
 template <bool FOLD>
 __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<double>& C,
                                                  double (&ox)[2], double (&oy)[2], double (&oz)[2]) {
+    uint32_t w0[2], w1[2], w2[2];
+    group_words<2>(g0, K, w0, w1, w2);
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-        uint32_t w0, w1, w2;
-        particle_words(g0 + (uint64_t)e, K, w0, w1, w2);
-        velocity_f64(w0, w1, w2, C, ox[e], oy[e], oz[e]);
-    }
+    for (int e = 0; e < 2; ++e) velocity_f64(w0[e], w1[e], w2[e], C, ox[e], oy[e], oz[e]);
 }
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
@@ -171,12 +186,18 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t offset, const __grid_const
 __global__ void __launch_bounds__(kThreads)
 words_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,
              uint32_t* __restrict__ o1, uint32_t* __restrict__ o2) {
-    for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
-        uint32_t w0, w1, w2;
-        particle_words(offset + (uint64_t)i, K, w0, w1, w2);
-        o0[i] = w0;
-        o1[i] = w1;
-        o2[i] = w2;
+    // four consecutive particles per thread through group_words, exactly as the fp32 sampler draws them
+    for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n; i += (int64_t)gridDim.x * kThreads * 4) {
+        uint32_t w0[4], w1[4], w2[4];
+        group_words<4>(offset + (uint64_t)i, K, w0, w1, w2);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (i + e < n) {
+                o0[i + e] = w0[e];
+                o1[i + e] = w1[e];
+                o2[i + e] = w2[e];
+            }
+        }
     }
 }
 

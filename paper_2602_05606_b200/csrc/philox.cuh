@@ -56,6 +56,42 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     w0 = c0; w1 = c1; w2 = c2; w3 = c3;
 }
 
+// Counters that share their high word.  With ctr = (c0, c1, 0, 0) round 1 multiplies M1 by zero, so
+// after it the new word 0 is c1 ^ k0[0] -- the same for every particle with the same hi32(g) -- and
+// round 2's product M0 * (c1 ^ k0[0]) is shared too.  A thread computes this head once per 128-bit
+// group and each particle then needs 18 wide multiplies instead of 19 (+1 shared) and no 64-bit add.
+struct PhiloxHead {
+    uint32_t hi, lo;   // M0 * (hi32(g) ^ k0[0])
+};
+__device__ __forceinline__ PhiloxHead philox_head(uint32_t g_hi, const PhiloxKeys& K) {
+    const uint64_t p = (uint64_t)kPhiloxM0 * (uint64_t)(g_hi ^ K.k0[0]);
+    return PhiloxHead{(uint32_t)(p >> 32), (uint32_t)p};
+}
+// Same words as particle_words(g, ...) for g = (g_hi << 32) | g_lo, given H = philox_head(g_hi, K).
+__device__ __forceinline__ void particle_words_head(uint32_t g_lo, const PhiloxHead& H, const PhiloxKeys& K,
+                                                    uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+    // round 1 (c2 = c3 = 0): c = (g_hi ^ k0[0], 0, hi(M0 g_lo) ^ k1[0], lo(M0 g_lo))
+    const uint64_t q0 = (uint64_t)kPhiloxM0 * (uint64_t)g_lo;
+    // round 2: the M0 product is the shared head; c1 = 0
+    const uint64_t q1 = (uint64_t)kPhiloxM1 * (uint64_t)((uint32_t)(q0 >> 32) ^ K.k1[0]);
+    uint32_t c0 = (uint32_t)(q1 >> 32) ^ K.k0[1];
+    uint32_t c1 = (uint32_t)q1;
+    uint32_t c2 = H.hi ^ (uint32_t)q0 ^ K.k1[1];
+    uint32_t c3 = H.lo;
+#pragma unroll
+    for (int r = 2; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    w0 = c0; w1 = c1; w2 = c2;
+}
+
 // The three words particle g consumes (w3 is drawn and discarded, reading R4).
 __device__ __forceinline__ void particle_words(uint64_t g, const PhiloxKeys& K, uint32_t& w0,
                                                uint32_t& w1, uint32_t& w2) {

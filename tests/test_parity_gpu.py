@@ -20,7 +20,7 @@ def ref_sample(n, kappa, theta, seed, offset=0):
 
 
 # ------------------------------------------------------------------ S1: words, bit-exact
-@pytest.mark.parametrize("seed,offset,n", [(0, 0, 1_000_000), (1, 0, 4097), (42, 2**32 - 1000, 2000),
+@pytest.mark.parametrize("seed,offset,n", [(0, 0, 1_000_000), (1, 0, 4097), (42, 2**32 - 1000, 2000), (42, 2**32 - 1001, 2003), (5, 2**32 - 3, 9),
                                            (123, 3 * 2**28 - 5, 4101), (0xA4093822_299F31D0, 2**40 + 7, 1000),
                                            (7, 2**64 - 500, 1000)])
 def test_words_bit_exact(seed, offset, n):
@@ -117,6 +117,18 @@ def test_theta_zero_and_status_codes():
     buf = torch.empty(64, dtype=torch.uint8, device="cuda")
     rc = kg.lib().kappagen_sample(4, 2.0, 1.0, 0, 0, kg.F64, buf.data_ptr() + 4, buf.data_ptr() + 8, buf.data_ptr() + 16, None)
     assert rc == kg.EALIGN
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("offset", [2**32 - 1001, 2**32 - 2, 2**33 - 6, 2**64 - 5])
+def test_sample_parity_across_counter_carry(dtype, offset):
+    """The low counter word wraps inside a 128-bit group (odd offsets): the sampler's shared-head Philox
+    must fall back to the per-particle counter there (64-bit carry, reading R6)."""
+    n = 2003
+    got = kg.sample(n, 2.5, 0.7, 9, offset, dtype)
+    want = ref_sample(n, 2.5, 0.7, 9, offset % 2**64)
+    err = max_rel_err(got, want)
+    assert err <= TOL[dtype], err
 
 
 # ------------------------------------------------------------------ chunk continuation (config 5, small and full)
