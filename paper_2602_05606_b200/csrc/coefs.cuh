@@ -6,7 +6,7 @@
 //   A    = a + cL            = a  - ck  * Y          ck  = c kappa*
 //   disc = (a+cL)^2 - 4bL    = A^2 + bk4 * Y         bk4 = 4 b kappa*
 //   x    = -2L / (A + sqrt(disc))   = k2 * Y / (A + D)     k2  = 2 kappa*      (A >= 0)
-//        = (-A + sqrt(disc)) / (2b) = (D - A) * i2b        i2b = 1/(2b)        (A <  0)
+//        = (-A + sqrt(disc)) / (2b) = (D - A) / b2         b2  = 2b            (A <  0)
 // (the two printed forms of Eq. (24)).  V = theta sqrt(x).
 #pragma once
 #include <cmath>
@@ -30,7 +30,7 @@ struct alignas(16) Coef<double> {
     double ck;     // c kappa*
     double bk4;    // 4 b kappa*
     double k2;     // 2 kappa*
-    double i2b;    // 1/(2b)
+    double b2;     // 2 b
     double theta;  // most probable speed; NaN marks an invalid cell
     double pad;
 };
@@ -100,7 +100,7 @@ KAPPAGEN_HD inline Coef<double> make_coef_f64(const TableIParams<F>& P, F theta)
     C.ck = (double)(P.c * P.kstar);
     C.bk4 = (double)(F(4.0) * P.b * P.kstar);
     C.k2 = (double)(F(2.0) * P.kstar);
-    C.i2b = (double)(F(1.0) / (F(2.0) * P.b));
+    C.b2 = (double)(F(2.0) * P.b);
     C.theta = (double)theta;
     C.pad = 0.0;
     return C;
