@@ -65,7 +65,7 @@ static int check_planes(const char* fn, int64_t n, int dtype, const void* vx, co
 template <typename T, bool VEC, bool FOLD>
 static int launch_sample_as(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T* vx, T* vy, T* vz,
                             cudaStream_t st) {
-    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * TileTraits<T>::groups;
     int grid = 0, rc;
     if ((rc = grid_for(sample_kernel<T, VEC, FOLD>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
     sample_kernel<T, VEC, FOLD><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);

@@ -18,6 +18,26 @@ namespace kappagen {
 
 constexpr int kThreads = 256;
 constexpr int kGroups = 2;  // 128-bit groups per thread per tile
+// Tile shape of the sample kernels, measured on B200 (_F64 macros are sweep knobs).
+// double: 4 groups (8 particles) per thread generated in one straight line -- whole tiles only, stores
+// last -- under __launch_bounds__(256, 2): the chains are long, latency-bound and share 64-bit constants,
+// and 122 registers let the compiler keep those constants resident (1.05e11 particles/s against 9.1e10
+// for 2 separate groups at 80 registers).  float: 2 groups, each generated and stored on its own (joint
+// generation costs registers and 3 %); min-blocks 1 spelled out lets ptxas use 54 registers (+1 %).
+#ifndef KG_JOINT_F64
+#define KG_JOINT_F64 1
+#endif
+#ifndef KG_F64_GROUPS
+#define KG_F64_GROUPS 4
+#endif
+#ifndef KG_F64_MINB
+#define KG_F64_MINB 2
+#endif
+template <typename T> struct TileTraits {
+    static constexpr bool joint = (sizeof(T) == 8) && KG_JOINT_F64;
+    static constexpr int groups = sizeof(T) == 8 ? KG_F64_GROUPS : kGroups;   // of the sample kernel
+    static constexpr int minb = sizeof(T) == 8 ? KG_F64_MINB : 1;
+};
 
 template <typename T> struct Vec128;
 template <> struct Vec128<float> { using type = float4; };
@@ -102,21 +122,51 @@ __device__ __forceinline__ void store_planes(int64_t i, int64_t n, T* __restrict
 }
 
 // ---------------------------------------------------------------- kappagen_sample
+// Group j of the tile at `base`, bounds-checked (ragged tail, unaligned planes).
 template <typename T, bool VEC, bool FOLD>
-__global__ void __launch_bounds__(kThreads)
+__device__ __forceinline__ void tile_group(int64_t base, int j, int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C,
+                                           T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    constexpr int G = 16 / sizeof(T);
+    const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+    if (i < n) {
+        T ox[G], oy[G], oz[G];
+        group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox, oy, oz);
+        store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+    }
+}
+
+template <typename T, bool VEC, bool FOLD>
+__global__ void __launch_bounds__(kThreads, TileTraits<T>::minb)
 sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
               T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     constexpr int G = 16 / sizeof(T);
-    constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    constexpr int NG = TileTraits<T>::groups;
+    constexpr int64_t kTile = (int64_t)kThreads * G * NG;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        if (VEC && TileTraits<T>::joint && base + kTile <= n) {
+            // whole tile in range: all groups of the thread in one straight line, so that their independent
+            // chains interleave and share the materialised constants; stores last
+            T ox[NG][G], oy[NG][G], oz[NG][G];
 #pragma unroll
-        for (int j = 0; j < kGroups; ++j) {
-            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
-            if (i < n) {
-                T ox[G], oy[G], oz[G];
-                group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox, oy, oz);
-                store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+            for (int j = 0; j < NG; ++j) {
+                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox[j], oy[j], oz[j]);
             }
+#pragma unroll
+            for (int j = 0; j < NG; ++j) {
+                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                store_group(vx + i, ox[j]);
+                store_group(vy + i, oy[j]);
+                store_group(vz + i, oz[j]);
+            }
+            continue;
+        }
+        if constexpr (TileTraits<T>::joint) {
+#pragma unroll 1
+            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD>(base, j, n, offset, K, C, vx, vy, vz);
+        } else {
+#pragma unroll
+            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD>(base, j, n, offset, K, C, vx, vy, vz);
         }
     }
 }

@@ -3,7 +3,8 @@
 // measured 6.3e-14.
 //
 // The chain is the cancellation-free re-association of DESIGN.md readings R3, R7:
-//   1 - U      exact, from the integer complement ~w          (PAPER.md:250 turned into an identity)
+//   1 - U      exact: U = (w + 1/2)/2^32 has 33 significant bits, so 1 - U is the double ((~w) + 1/2)/2^32
+//              (PAPER.md:250 turned into an identity)
 //   1 - U1^(2/3) = t1 (1+r)/(1+r+r^2),  r = cbrt(U1), t1 = 1-U1   (since 1 - r^3 = t1)
 //   (..)^(-1/kappa*) - 1 = expm1(-ln(S)/kappa*)
 //   root of Eq. (24): the printed form whose denominator/numerator adds
@@ -38,9 +39,10 @@ __device__ __forceinline__ double u32_affine(uint32_t w, double scale, double bi
 __device__ __forceinline__ float seed_in(double x) {
     return __uint_as_float(((uint32_t)__double2hiint(x) << 3) + 0x40000000u);   // (hi - 0x38000000) << 3
 }
-// double view of a positive float: 20 mantissa bits kept (relative error < 2^-20 in total, by design).
+// double view of a positive float: 20 mantissa bits kept; the low word is don't-care (< 2^-20 relative)
+// and reuses the float's register so that no zero has to be materialised.
 __device__ __forceinline__ double seed_out(float s) {
-    return __hiloint2double((int)((__float_as_uint(s) >> 3) + 0x38000000u), 0);
+    return __hiloint2double((int)((__float_as_uint(s) >> 3) + 0x38000000u), (int)__float_as_uint(s));
 }
 
 // 1/d, third order: e = 1 - d z0, z = z0 (1 + e + e^2).
@@ -65,7 +67,7 @@ __device__ __forceinline__ double rsqrt3_f64(double z) {
 
 __device__ __forceinline__ double speed_f64(uint32_t w0, const Coef<double>& C) {
     const double u1 = u32_affine(w0, 0x1p-32, -0x1p20 + 0x1p-33);               // U1 = (w0 + 1/2)/2^32, exact
-    const double t1 = u32_affine(~w0, 0x1p-32, -0x1p20 + 0x1p-33);              // 1 - U1, exact
+    const double t1 = 1.0 - u1;                                                  // exact: U1 has 33 significant bits
     // y = U1^(-1/3): fp32 seed 2^((32 - log2(w0 + 1/2))/3), then e = 1 - u y0^3, y = y0 (1 + e/3 + 2 e^2/9)
     float lg, ys;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"((float)w0 + 0.5f));
@@ -125,7 +127,7 @@ __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t 
                                              const Coef<double>& C, double& vx, double& vy, double& vz) {
     const double V = speed_f64(w0, C);
     const double u2 = u32_affine(w1, 0x1p-32, -0x1p20 + 0x1p-33);               // U2, exact
-    const double t2 = u32_affine(~w1, 0x1p-32, -0x1p20 + 0x1p-33);              // 1 - U2, exact
+    const double t2 = 1.0 - u2;                                                  // 1 - U2, exact
     const double mu = u2 - t2;                                                   // 2 U2 - 1, exact
     const double zz = u2 * t2;
     const double sth = zz * rsqrt3_f64(zz);                                      // sqrt(U2 (1-U2)); the 2 goes into Vs
