@@ -31,9 +31,20 @@ KAPPA, THETA, SEED = 2.0, 0.1, 42
 REF_SAMPLE = 1 << 20                   # particles per step of the --impl reference arm
 CPU_BASELINE_SAMPLE = 1 << 24          # particles of the cpu_baseline leg (~10-20 s of one core)
 FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum of one sample_kernel launch at 2^28 particles, from the
-# ncu --set full capture summarised in profiles/ (None until a capture exists for that dtype).
-NCU_TRAFFIC_BYTES = {"f32": None, "f64": None}
+FALLBACK_SM_MHZ = 1965.0               # B200 maximum SM clock (MEASURED_PEAKS.json sm_max_mhz when present)
+N_SM = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of one sample_kernel launch at 2^28 particles, and the busy
+# fraction of the limiting pipe, from the ncu --set full captures summarised in profiles/r01c_kernels.md.
+NCU_TRAFFIC_BYTES = {"f32": 3162542408, "f64": 6383231288}
+NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed", 79.2),
+                "f64": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 57.5)}
+# The sampler is bound by SM arithmetic, not by HBM.  Algorithmic work per particle on
+# the limiting pipe and that pipe's peak rate in thread-operations per clock per SM:
+#   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a
+#        quarter of the 128-lane FMA rate on sm_100 (measured 31.5 per clock per SM) -> 32 /clk/SM.
+#   f64: the double chain is 99 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
+ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
+            "f64": (99, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
 
 
 def parse_args():
@@ -226,7 +237,16 @@ def run_ours(args):
                 peak, which = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
         except Exception:
             pass
-        achieved = 3 * es * n / (kern_ms * 1e-3) / 1e9
+        hbm_achieved = 3 * es * n / (kern_ms * 1e-3) / 1e9
+        sm_mhz = FALLBACK_SM_MHZ
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                sm_mhz = float(json.load(f)["sm_max_mhz"])
+        except Exception:
+            pass
+        ops, per_clk, alu_unit, pipe = ALU_WORK[dtype]
+        alu_achieved = ops * n / (kern_ms * 1e-3) / 1e9
+        alu_peak = N_SM * per_clk * sm_mhz * 1e6 / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -234,10 +254,14 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": args.steps,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 3 * es * n * world,
                     "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES[dtype], "peak_source": which, "kernel": "sample_kernel<%s,true>" % dtype,
-                         "algorithmic_bytes_per_launch": 3 * es * n, "kernel_ms": kern_ms,
-                         "kernel_ms_min": min(per_launch), "kernel_ms_max": max(per_launch)},
+            "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": alu_unit,
+                         "frac": alu_achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES[dtype], "pipe": pipe,
+                         "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5)" % (N_SM, per_clk, sm_mhz),
+                         "algorithmic_ops_per_particle": ops, "kernel": "sample_kernel<%s>" % dtype,
+                         "kernel_ms": kern_ms, "kernel_ms_min": min(per_launch), "kernel_ms_max": max(per_launch),
+                         "ncu_pipe_busy_pct": {NCU_PIPE_PCT[dtype][0]: NCU_PIPE_PCT[dtype][1]},
+                         "hbm": {"achieved": hbm_achieved, "peak": peak, "unit": "GB/s", "frac": hbm_achieved / peak,
+                                 "algorithmic_bytes_per_launch": 3 * es * n, "peak_source": which}},
         }
         if world == 1 and not args.no_extras:
             line["extras"] = extras(kg, torch, dtype)
