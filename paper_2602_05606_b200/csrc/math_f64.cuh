@@ -64,26 +64,37 @@ __device__ __forceinline__ double rsqrt3_f64(double z) {
     const double q = fma(e, 0.375, 0.5);
     return fma(g0, q * e, g0);
 }
+// sqrt(z) by the same correction applied to t = z g0 (one multiply fewer than z * rsqrt3_f64(z)).
+__device__ __forceinline__ double sqrt3_f64(double z) {
+    float s;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(seed_in(z)));
+    const double g0 = seed_out(s);
+    const double t = z * g0;
+    const double e = fma(-t, g0, 1.0);
+    const double q = fma(e, 0.375, 0.5);
+    return fma(t, q * e, t);
+}
 
 __device__ __forceinline__ double speed_f64(uint32_t w0, const Coef<double>& C) {
     const double u1 = u32_affine(w0, 0x1p-32, -0x1p20 + 0x1p-33);               // U1 = (w0 + 1/2)/2^32, exact
     const double t1 = 1.0 - u1;                                                  // exact: U1 has 33 significant bits
-    // y = U1^(-1/3): fp32 seed 2^((32 - log2(w0 + 1/2))/3), then e = 1 - u y0^3, y = y0 (1 + e/3 + 2 e^2/9)
+    // r = U1^(1/3): fp32 seed y0 ~ U1^(-1/3) = 2^((32 - log2(w0 + 1/2))/3); r0 = u y0^2, e = 1 - u y0^3 = 1 - r0 y0,
+    // r = u y^2 with y = y0 (1-e)^(-1/3):  r = r0 (1 + 2e/3 + 5e^2/9), residual ~ e^3
     float lg, ys;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"((float)w0 + 0.5f));
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ys) : "f"(fmaf(lg, -0x1.555556p-2f, 0x1.555556p+3f)));
     const double y0 = seed_out(ys);
-    const double e = fma(-(y0 * y0) * u1, y0, 1.0);
-    const double y = fma(y0, fma(e, 0x1.c71c71c71c71cp-3, 0x1.5555555555555p-2) * e, y0);
-    const double r = u1 * (y * y);                                               // U1^(1/3)
+    const double r0 = (y0 * y0) * u1;
+    const double e = fma(-r0, y0, 1.0);
+    const double r = fma(r0, fma(e, 0x1.1c71c71c71c72p-1, 0x1.5555555555555p-1) * e, r0);   // 5/9, 2/3
     const double p = r * r;                                                      // U1^(2/3)
     const double q1 = 1.0 + r;
     const double S = (t1 * q1) * rcp3_f64(q1 + p);                               // 1 - U1^(2/3), no cancellation
-    // ln S = k ln2 + 2 f P(f^2), S = 2^k m, m in [sqrt(1/2), sqrt(2)); p < 0.29 implies k = 0, m = S
+    // ln S = k ln2 + 2 f P(f^2), S = 2^k m, m in [sqrt(1/2), sqrt(2)); S < 1 so k <= 0
     const int hi = __double2hiint(S);
     const int k = (hi - 0x3fe6a09e) >> 20;
     const double m = __hiloint2double(hi - (k << 20), __double2loint(S));
-    const double num = (p < 0.29) ? -p : m - 1.0;                                // m - 1 = -p exactly where S -> 1
+    const double num = (k == 0) ? -p : m - 1.0;                                  // k = 0: m - 1 = S - 1 = -p, without cancellation
     const double f = num * rcp3_f64(num + 2.0);
     const double z = f * f;
     double P = 0x1.58dde2537d4c5p-4;
@@ -115,7 +126,7 @@ __device__ __forceinline__ double speed_f64(uint32_t w0, const Coef<double>& C) 
     // Eq. (24): root of b x^2 + A x - kappa* Y = 0, A = a + cL = a - c kappa* Y, in the form that adds
     const double A = fma(-C.ck, Y, C.a);
     const double disc = fma(A, A, C.bk4 * Y);                                    // (a+cL)^2 - 4bL > A^2
-    const double T = fabs(A) + disc * rsqrt3_f64(disc);                          // |A| + sqrt(disc)
+    const double T = fabs(A) + sqrt3_f64(disc);                                  // |A| + sqrt(disc)
     // x = num/den:  A >= 0: 2 kappa* Y / T;   A < 0: T / (2b).   V = theta sqrt(num/den) = theta num / sqrt(num den)
     const bool pos = A >= 0.0;
     const double nm = pos ? C.k2 * Y : T;
@@ -130,7 +141,7 @@ __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t 
     const double t2 = 1.0 - u2;                                                  // 1 - U2, exact
     const double mu = u2 - t2;                                                   // 2 U2 - 1, exact
     const double zz = u2 * t2;
-    const double sth = zz * rsqrt3_f64(zz);                                      // sqrt(U2 (1-U2)); the 2 goes into Vs
+    const double sth = sqrt3_f64(zz);                                            // sqrt(U2 (1-U2)); the 2 goes into Vs
     // 2 pi U3 = (pi/2)(k + q): k = nearest quarter turn, q = ((int32)(w2 << 2) + 2)/2^32 in (-1/2, 1/2)
     const double q = u32_affine((w2 << 2) ^ 0x80000000u, 0x1p-32, -0x1p20 - 0.5 + 0x1p-31);
     const double z = q * q;
