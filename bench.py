@@ -42,9 +42,9 @@ NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustain
 # the limiting pipe and that pipe's peak rate in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a
 #        quarter of the 128-lane FMA rate on sm_100 (measured 31.5 per clock per SM) -> 32 /clk/SM.
-#   f64: the double chain is 99 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
+#   f64: the double chain is 95 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
-            "f64": (99, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+            "f64": (95, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
 
 
 def parse_args():
@@ -293,6 +293,18 @@ def extras(kg, torch, dtype):
         _, ms = time_launches(lambda s: kg.baseline_mt(n, KAPPA, THETA, SEED, s * n, dt, out=planes[dt], stream=st), 5, 2, torch)
         k = sum(ms) / len(ms)
         out["baseline_mt_" + dt] = {"particles_per_s": n / (k * 1e-3), "kernel_ms": k, "write_GBps": 3 * es[dt] * n / (k * 1e-3) / 1e9}
+    # configs[3]: PIC-style per-cell parameters, 256x256x64 cells x 64 particles (pre-kernel + sampling kernel)
+    from paper_2602_05606_b200 import workloads as wl
+    cfg = wl.C4
+    kap, th = wl.cell_arrays(cfg)
+    kd, td = torch.from_numpy(kap).cuda(), torch.from_numpy(th).cuda()
+    dd = torch.tensor(cfg.drift, dtype=torch.float32, device="cuda")
+    ws = torch.empty(kg.cells_workspace_bytes(cfg.ncell, "f32"), dtype=torch.uint8, device="cuda")
+    nc = cfg.ncell * cfg.ppc
+    _, ms = time_launches(lambda s: kg.sample_cells(cfg.ppc, kd, td, dd, 0, cfg.seed, s * nc, out=p32, workspace=ws, stream=st),
+                          5, 2, torch)
+    k = sum(ms) / len(ms)
+    out["sample_cells_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k, "write_GBps": 12 * nc / (k * 1e-3) / 1e9}
     return out
 
 

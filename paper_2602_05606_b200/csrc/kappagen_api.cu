@@ -116,12 +116,15 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
     const int64_t tiles = (n + tile - 1) / tile;
     int grid = 0, rc;
+    // floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1) for every i with i * ppc < 2^64 (i < n)
+    const uint64_t up = (uint64_t)ppc;
+    const uint64_t magic = (up >= 2 && (uint64_t)n <= (~0ull) / up) ? (~0ull) / up + 1 : 0;
     if (vec) {
         if ((rc = grid_for(sample_cells_kernel<T, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_cells_kernel<T, true><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, offset, K, W, drift, drift_stride, vx, vy, vz);
+        sample_cells_kernel<T, true><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz);
     } else {
         if ((rc = grid_for(sample_cells_kernel<T, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_cells_kernel<T, false><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, offset, K, W, drift, drift_stride, vx, vy, vz);
+        sample_cells_kernel<T, false><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz);
     }
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;

@@ -196,9 +196,25 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
     W[cell] = C;
 }
 
+// floor(i / ppc) without a 64-bit division: magic = floor(2^64 / ppc) + 1 is exact for i * ppc < 2^64 (the
+// launcher checks n * ppc < 2^64 and passes magic = 0 otherwise, which selects the plain division).
+__device__ __forceinline__ int64_t cell_of(int64_t i, uint32_t ppc, uint64_t magic) {
+    return magic ? (int64_t)__umul64hi((uint64_t)i, magic) : i / (int64_t)ppc;
+}
+
+template <typename T>
+__device__ __forceinline__ void add_drift(const T* __restrict__ d, T& x, T& y, T& z) {
+    x += d[0];
+    y += d[1];
+    z += d[2];
+}
+
+// Particle g = cell * ppc + j (cell-major).  A 128-bit group of G particles that lies inside one cell -- every
+// group when ppc is a multiple of G -- loads that cell's Coef<T> once and runs the same packed / shared-head
+// code as the uniform sampler; a group that straddles a cell boundary takes the per-particle path.
 template <typename T, bool VEC>
 __global__ void __launch_bounds__(kThreads)
-sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t offset, const __grid_constant__ PhiloxKeys K,
+sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, const __grid_constant__ PhiloxKeys K,
                     const Coef<T>* __restrict__ W, const T* __restrict__ drift, int64_t drift_stride,
                     T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     constexpr int G = 16 / sizeof(T);
@@ -208,22 +224,32 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t offset, const __grid_const
         for (int j = 0; j < kGroups; ++j) {
             const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
             if (i < n) {
-                const int64_t cell0 = i / (int64_t)ppc;
+                const int64_t cell0 = cell_of(i, ppc, magic);
                 const uint32_t rem = (uint32_t)(i - cell0 * (int64_t)ppc);
                 T ox[G], oy[G], oz[G];
-#pragma unroll
-                for (int e = 0; e < G; ++e) {
-                    int64_t cell = cell0 + (int64_t)((rem + (uint32_t)e) / ppc);
-                    if (i + e >= n) cell = cell0;                     // lanes past the end: stay in bounds
-                    const Coef<T> C = W[cell];
-                    uint32_t w0, w1, w2;
-                    particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                    velocity<false>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                if (rem + (uint32_t)G <= ppc && i + G <= n) {
+                    const Coef<T> C = W[cell0];
+                    group_velocities<false>(offset + (uint64_t)i, K, C, ox, oy, oz);
                     if (drift != nullptr) {
-                        const T* d = drift + 3 * cell * drift_stride;
-                        ox[e] += d[0];
-                        oy[e] += d[1];
-                        oz[e] += d[2];
+                        const T* d = drift + 3 * cell0 * drift_stride;
+                        const T dx = d[0], dy = d[1], dz = d[2];
+#pragma unroll
+                        for (int e = 0; e < G; ++e) {
+                            ox[e] += dx;
+                            oy[e] += dy;
+                            oz[e] += dz;
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < G; ++e) {
+                        int64_t cell = cell0 + (int64_t)((rem + (uint32_t)e) / ppc);
+                        if (i + e >= n) cell = cell0;                 // lanes past the end: stay in bounds
+                        const Coef<T> C = W[cell];
+                        uint32_t w0, w1, w2;
+                        particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
+                        velocity<false>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                        if (drift != nullptr) add_drift(drift + 3 * cell * drift_stride, ox[e], oy[e], oz[e]);
                     }
                 }
                 store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
