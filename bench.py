@@ -42,9 +42,9 @@ NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustain
 # the limiting pipe and that pipe's peak rate in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a
 #        quarter of the 128-lane FMA rate on sm_100 (measured 31.5 per clock per SM) -> 32 /clk/SM.
-#   f64: the double chain is 95 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
+#   f64: the double chain is 96 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
-            "f64": (95, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+            "f64": (96, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
 
 
 def parse_args():
