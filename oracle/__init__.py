@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
             L.oracle_sample_cells.argtypes = [i64, i32, _f64p, _f64p, _f64p, i64, u64, u64,
                                               _f64p, _f64p, _f64p, _f64p, _f64p, _f64p]
             L.oracle_sample_cells.restype = ctypes.c_int
+            L.oracle_cells_moments.argtypes = [i64, i32, _f64p, _f64p, _f64p, i64, u64, u64, _f64p, _f64p]
+            L.oracle_cells_moments.restype = ctypes.c_int
             L.oracle_version.restype = ctypes.c_int
             _lib = L
     return _lib
@@ -168,3 +170,23 @@ def sample_cells(ppc: int, kappa, theta, drift, drift_stride: int, seed: int, of
     if rc != 0:
         raise ValueError("bad arguments")
     return (tuple(v), tuple(t)) if thermal else tuple(v)
+
+
+def cells_moments(ppc: int, kappa, theta, drift, drift_stride: int, seed: int, offset: int = 0):
+    """Per-cell (sum vx, sum vy, sum vz, sum |v|^2) of sample_cells' particles, drift included, and the
+    per-cell sum of |vx|+|vy|+|vz| (the scale of the admissible rounding error).  Returns (mom[ncell,4], abs1)."""
+    kappa = np.ascontiguousarray(kappa, dtype=np.float64)
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    ncell = kappa.size
+    mom = np.empty((ncell, 4), dtype=np.float64)
+    abs1 = np.empty(ncell, dtype=np.float64)
+    null = ctypes.cast(None, _f64p)
+    dptr = null
+    if drift is not None:
+        drift = np.ascontiguousarray(drift, dtype=np.float64)
+        dptr = _p64(drift)
+    rc = lib().oracle_cells_moments(ncell, ppc, _p64(kappa), _p64(theta), dptr, drift_stride, seed, offset,
+                                    _p64(mom), _p64(abs1))
+    if rc != 0:
+        raise ValueError("bad arguments")
+    return mom, abs1

@@ -315,6 +315,38 @@ int oracle_sample_cells(int64_t ncell, int32_t ppc, const double* kappa, const d
     return 0;
 }
 
+// Per-cell velocity moments of the same particles (the fused loader of SURVEY.md section 8(f) f1: what a
+// PIC code computes right after loading -- momentum and the energy density of Eq. (5)):
+//   mom[4*cell + 0..2] = sum_j (vx, vy, vz),   mom[4*cell + 3] = sum_j (vx^2 + vy^2 + vz^2)
+// over the cell's ppc particles, drift included, accumulated in long double and rounded once.  abs1
+// (optional) receives sum_j (|vx| + |vy| + |vz|) per cell, the scale of the admissible rounding error.
+int oracle_cells_moments(int64_t ncell, int32_t ppc, const double* kappa, const double* theta,
+                         const double* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                         double* mom, double* abs1) {
+    if (ncell < 0 || ppc < 0) return -1;
+    for (int64_t cell = 0; cell < ncell; ++cell) {
+        const bool ok = params_ok(kappa[cell], theta[cell]);
+        Params P = {};
+        if (ok) P = params_of((ld)kappa[cell]);
+        ld d3[3] = {0.0L, 0.0L, 0.0L};
+        if (drift) for (int q = 0; q < 3; ++q) d3[q] = (ld)drift[3 * cell * drift_stride + q];
+        ld s[4] = {0.0L, 0.0L, 0.0L, 0.0L}, a1 = 0.0L;
+        for (int32_t j = 0; j < ppc; ++j) {
+            const int64_t i = cell * (int64_t)ppc + j;
+            if (!ok) { s[0] = s[1] = s[2] = s[3] = a1 = (ld)NAN; break; }
+            uint32_t w[4];
+            particle_words(seed, offset + (uint64_t)i, w);
+            const ld V = (ld)theta[cell] * sqrtl(x_stable(w[0], P));
+            const Dir d = dir_stable(w[1], w[2]);
+            const ld v3[3] = {V * d.mu + d3[0], V * d.sth * d.cphi + d3[1], V * d.sth * d.sphi + d3[2]};
+            for (int q = 0; q < 3; ++q) { s[q] += v3[q]; s[3] += v3[q] * v3[q]; a1 += fabsl(v3[q]); }
+        }
+        for (int q = 0; q < 4; ++q) mom[4 * cell + q] = (double)s[q];
+        if (abs1) abs1[cell] = (double)a1;
+    }
+    return 0;
+}
+
 int oracle_version(void) { return 1; }
 
 }  // extern "C"
