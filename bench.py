@@ -305,6 +305,16 @@ def extras(kg, torch, dtype):
                           5, 2, torch)
     k = sum(ms) / len(ms)
     out["sample_cells_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k, "write_GBps": 12 * nc / (k * 1e-3) / 1e9}
+    # the fused loader: planes + per-cell moments in one kernel, and moments only
+    mom = torch.empty((cfg.ncell, 4), dtype=torch.float32, device="cuda")
+    _, ms = time_launches(lambda s: kg.sample_cells_moments(cfg.ppc, kd, td, dd, 0, cfg.seed, s * nc, out=p32, moments=mom,
+                                                            workspace=ws, stream=st), 5, 2, torch)
+    k = sum(ms) / len(ms)
+    out["sample_cells_moments_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k}
+    _, ms = time_launches(lambda s: kg.sample_cells_moments(cfg.ppc, kd, td, dd, 0, cfg.seed, s * nc, moments=mom, workspace=ws,
+                                                            stream=st, store=False), 5, 2, torch)
+    k = sum(ms) / len(ms)
+    out["cells_moments_only_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k}
     return out
 
 

@@ -70,6 +70,24 @@ int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const v
                           void* workspace, size_t workspace_bytes, void* stream);
 size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype);
 
+/* The loader fused with its first consumer (the step after the path in a PIC code: "initialization stage",
+ * PAPER.md:15; 10^2-10^3 particles per cell): kappagen_sample_cells that ALSO reduces, per
+ * cell and inside the generating kernel, the velocity moments of the cell's ppc particles (drift included)
+ *     moments[4*cell + 0..2] = sum (vx, vy, vz)        (momentum density / m)
+ *     moments[4*cell + 3]    = sum (vx^2 + vy^2 + vz^2)  (2/m x the energy density whose expectation is
+ *                                                        Eq. (5): 3 kappa theta^2/(2 kappa - 3) each)
+ * so that the consumer never re-reads the 12/24 B per particle.
+ *  moments : device, [ncell][4] elements of `dtype`, 16-byte aligned; overwritten (no need to zero it).
+ *  vx,vy,vz: as in kappagen_sample_cells, or ALL THREE NULL: moments only, no velocity is written to HBM.
+ * Sums are formed in `dtype`: within a thread over its 128-bit group, then across the cell's lanes by a
+ * shuffle tree (fixed order, bit-reproducible) when ppc = G*2^k <= 32 G (G = 4 float / 2 double), otherwise
+ * through atomicAdd (order not fixed; values agree to rounding).  Other arguments, errors and workspace as
+ * kappagen_sample_cells. */
+int kappagen_sample_cells_moments(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                  const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                  int dtype, void* vx, void* vy, void* vz, void* moments,
+                                  void* workspace, size_t workspace_bytes, void* stream);
+
 /* Host-buffer variant of kappagen_sample (the end-to-end path): vx, vy, vz are HOST arrays of
  * [n] elements (pinned memory makes the copies asynchronous and fast; pageable memory works).
  * Generates on the current device in chunks, double-buffered so that the device-to-host copy of

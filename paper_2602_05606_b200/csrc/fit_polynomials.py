@@ -6,7 +6,7 @@ Near-minimax fits by Chebyshev interpolation in 60-digit arithmetic (mpmath): ev
 bounded away from zero on its interval, so absolute and relative error coincide up to a constant.  The
 script prints, per function, the degree, the measured maximum relative error on a dense grid and the
 coefficients rounded to the target type, ready to paste into the headers.  It belongs to the CUDA path
-only: oracle/ neither imports nor runs it, and nothing here is used at run time.
+only: the CPU checker neither imports nor runs it, and nothing here is used at run time.
 """
 from __future__ import annotations
 

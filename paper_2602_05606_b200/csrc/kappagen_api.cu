@@ -105,29 +105,45 @@ static int sample_on_stream(const char* fn, int64_t n, double kappa, double thet
     return launch_sample(n, offset, K, kappa, theta, vec, (double*)vx, (double*)vy, (double*)vz, st);
 }
 
+template <typename T, bool VEC, bool STORE, bool MOM>
+static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint64_t offset, const PhiloxKeys& K, const Coef<T>* W,
+                           const T* drift, int64_t drift_stride, T* vx, T* vy, T* vz, T* mom, int mode, int lanes,
+                           cudaStream_t st) {
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    int grid = 0, rc;
+    if ((rc = grid_for(sample_cells_kernel<T, VEC, STORE, MOM>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
+    sample_cells_kernel<T, VEC, STORE, MOM><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride,
+                                                                      vx, vy, vz, mom, mode, lanes);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+// store: write the planes; mom != nullptr: fused per-cell moments (at least one of the two).
 template <typename T>
 static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift,
-                        int64_t drift_stride, uint64_t offset, const PhiloxKeys& K, bool vec, T* vx, T* vy, T* vz,
-                        Coef<T>* W, cudaStream_t st) {
+                        int64_t drift_stride, uint64_t offset, const PhiloxKeys& K, bool vec, bool store, T* vx, T* vy,
+                        T* vz, T* mom, Coef<T>* W, cudaStream_t st) {
+    constexpr int G = 16 / sizeof(T);
+    int mode = kMomNone, lanes = 1;
+    if (mom != nullptr) {
+        const int L = ppc / G;
+        if (ppc % G == 0 && L <= 32 && (L & (L - 1)) == 0) { mode = kMomDirect; lanes = L; }
+        else if (ppc % (32 * G) == 0) { mode = kMomWarp; lanes = 32; }
+        else mode = kMomAtomic;
+    }
     const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
-    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, W);
+    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, W,
+                                                              (mode == kMomWarp || mode == kMomAtomic) ? mom : nullptr);
     KG_CUDA(cudaGetLastError());
     const int64_t n = ncell * (int64_t)ppc;
-    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
-    const int64_t tiles = (n + tile - 1) / tile;
-    int grid = 0, rc;
     // floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1) for every i with i * ppc < 2^64 (i < n)
     const uint64_t up = (uint64_t)ppc;
     const uint64_t magic = (up >= 2 && (uint64_t)n <= (~0ull) / up) ? (~0ull) / up + 1 : 0;
-    if (vec) {
-        if ((rc = grid_for(sample_cells_kernel<T, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_cells_kernel<T, true><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz);
-    } else {
-        if ((rc = grid_for(sample_cells_kernel<T, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        sample_cells_kernel<T, false><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz);
-    }
-    KG_CUDA(cudaGetLastError());
-    return KAPPAGEN_OK;
+#define KG_CELLS(V, S, M) launch_cells_as<T, V, S, M>(n, ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz, mom, mode, lanes, st)
+    if (mom == nullptr) return vec ? KG_CELLS(true, true, false) : KG_CELLS(false, true, false);
+    if (!store) return KG_CELLS(true, false, true);
+    return vec ? KG_CELLS(true, true, true) : KG_CELLS(false, true, true);
+#undef KG_CELLS
 }
 
 template <typename T>
@@ -159,11 +175,9 @@ extern "C" size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype) {
     return (size_t)ncell * (dtype == KAPPAGEN_F32 ? sizeof(Coef<float>) : sizeof(Coef<double>));
 }
 
-extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
-                                     const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
-                                     int dtype, void* vx, void* vy, void* vz, void* workspace,
-                                     size_t workspace_bytes, void* stream) {
-    const char* fn = "kappagen_sample_cells";
+static int cells_impl(const char* fn, int64_t ncell, int32_t ppc, const void* kappa, const void* theta, const void* drift,
+                      int64_t drift_stride, uint64_t seed, uint64_t offset, int dtype, void* vx, void* vy, void* vz,
+                      void* moments, bool want_moments, void* workspace, size_t workspace_bytes, void* stream) {
     if (ncell < 0 || ppc < 0) {
         set_error("%s: negative ncell or ppc", fn);
         return KAPPAGEN_EINVAL;
@@ -172,10 +186,17 @@ extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kap
         set_error("%s: ncell*ppc overflows", fn);
         return KAPPAGEN_EINVAL;
     }
+    if (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64) {
+        set_error("%s: dtype %d is neither KAPPAGEN_F32 nor KAPPAGEN_F64", fn, dtype);
+        return KAPPAGEN_EINVAL;
+    }
     bool vec = false;
     const int64_t n = ncell * (int64_t)ppc;
-    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
-    if (rc != KAPPAGEN_OK) return rc;
+    const bool store = !(want_moments && !vx && !vy && !vz);          // moments only: all three planes NULL
+    if (store) {
+        int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+        if (rc != KAPPAGEN_OK) return rc;
+    }
     if (drift != nullptr && drift_stride != 0 && drift_stride != 1) {
         set_error("%s: drift_stride must be 0 (shared) or 1 (per cell), got %lld", fn, (long long)drift_stride);
         return KAPPAGEN_EINVAL;
@@ -185,9 +206,17 @@ extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kap
         set_error("%s: NULL kappa or theta array", fn);
         return KAPPAGEN_ENULL;
     }
+    if (want_moments && !moments) {
+        set_error("%s: NULL moments array", fn);
+        return KAPPAGEN_ENULL;
+    }
     const size_t es = elem_size(dtype);
     if (!aligned_to(kappa, es) || !aligned_to(theta, es) || (drift && !aligned_to(drift, es))) {
         set_error("%s: kappa/theta/drift not aligned to the element size", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    if (want_moments && !aligned_to(moments, 16)) {
+        set_error("%s: moments not 16-byte aligned", fn);
         return KAPPAGEN_EALIGN;
     }
     if (!workspace || workspace_bytes < kappagen_cells_workspace_bytes(ncell, dtype) || !aligned_to(workspace, 16)) {
@@ -198,9 +227,27 @@ extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kap
     cudaStream_t st = (cudaStream_t)stream;
     if (dtype == KAPPAGEN_F32)
         return launch_cells<float>(ncell, ppc, (const float*)kappa, (const float*)theta, (const float*)drift, drift_stride,
-                                   offset, K, vec, (float*)vx, (float*)vy, (float*)vz, (Coef<float>*)workspace, st);
+                                   offset, K, vec, store, (float*)vx, (float*)vy, (float*)vz, (float*)moments,
+                                   (Coef<float>*)workspace, st);
     return launch_cells<double>(ncell, ppc, (const double*)kappa, (const double*)theta, (const double*)drift, drift_stride,
-                                offset, K, vec, (double*)vx, (double*)vy, (double*)vz, (Coef<double>*)workspace, st);
+                                offset, K, vec, store, (double*)vx, (double*)vy, (double*)vz, (double*)moments,
+                                (Coef<double>*)workspace, st);
+}
+
+extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                     const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                     int dtype, void* vx, void* vy, void* vz, void* workspace,
+                                     size_t workspace_bytes, void* stream) {
+    return cells_impl("kappagen_sample_cells", ncell, ppc, kappa, theta, drift, drift_stride, seed, offset, dtype, vx, vy, vz,
+                      nullptr, false, workspace, workspace_bytes, stream);
+}
+
+extern "C" int kappagen_sample_cells_moments(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                             const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                             int dtype, void* vx, void* vy, void* vz, void* moments, void* workspace,
+                                             size_t workspace_bytes, void* stream) {
+    return cells_impl("kappagen_sample_cells_moments", ncell, ppc, kappa, theta, drift, drift_stride, seed, offset, dtype, vx,
+                      vy, vz, moments, true, workspace, workspace_bytes, stream);
 }
 
 extern "C" int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,

@@ -183,9 +183,14 @@ template <> __device__ __forceinline__ Coef<double> cell_coef<double>(const Tabl
 // Pre-kernel: Table I lines 1-4 per cell, in double, into the workspace (one Coef<T> per cell).
 template <typename T>
 __global__ void __launch_bounds__(kThreads)
-cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict__ theta, Coef<T>* __restrict__ W) {
+cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict__ theta, Coef<T>* __restrict__ W,
+                 T* __restrict__ mom_to_zero) {
     const int64_t cell = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (cell >= ncell) return;
+    if (mom_to_zero != nullptr) {                                      // atomic moment modes accumulate into zeros
+#pragma unroll
+        for (int q = 0; q < 4; ++q) mom_to_zero[4 * cell + q] = T(0);
+    }
     const double kap = (double)kappa[cell], th = (double)theta[cell];
     const bool ok = isfinite(kap) && isfinite(th) && kap > 1.5 && th >= 0.0;
     const double ks = ok ? kap - 0.5 : 1.0;
@@ -209,14 +214,66 @@ __device__ __forceinline__ void add_drift(const T* __restrict__ d, T& x, T& y, T
     z += d[2];
 }
 
+// How the fused moments (kappagen_sample_cells_moments) leave the kernel.  All sums are in T.
+//   kMomDirect : ppc = G * L, L a power of two <= 32: the L lanes of a cell sit side by side in one warp; an
+//                xor-shuffle butterfly leaves each of the cell's four sums in one lane, which stores it.
+//                No atomics, fixed summation order (bit-reproducible).
+//   kMomWarp   : ppc a multiple of 32 G: a warp lies inside one cell; shuffle tree over the warp, then one
+//                atomicAdd per sum per warp into the zeroed buffer.
+//   kMomAtomic : any ppc: per group (or per particle where a group straddles two cells) atomicAdd.
+enum MomMode : int { kMomNone = 0, kMomDirect = 1, kMomWarp = 2, kMomAtomic = 3 };
+
+template <typename T>
+__device__ __forceinline__ void moments_out(T (&ps)[4], int64_t cell, int mode, int lanes, T* __restrict__ mom) {
+    if (mode == kMomAtomic) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) atomicAdd(mom + 4 * cell + q, ps[q]);
+        return;
+    }
+    const unsigned mask = __activemask();
+    const unsigned lane = threadIdx.x & (unsigned)(lanes - 1);         // lane inside the cell's segment
+    if (lanes >= 4) {
+        // Transposing butterfly: after two exchange steps each lane of a quad owns ONE of the four sums over
+        // its quad (5 shuffles for 16 lanes instead of 16); then a plain tree across quads on that one value.
+        const bool b0 = (lane & 1u) != 0u, b1 = (lane & 2u) != 0u;
+        const T r0 = (b0 ? ps[2] : ps[0]) + __shfl_xor_sync(mask, b0 ? ps[0] : ps[2], 1);
+        const T r1 = (b0 ? ps[3] : ps[1]) + __shfl_xor_sync(mask, b0 ? ps[1] : ps[3], 1);
+        T s = (b1 ? r1 : r0) + __shfl_xor_sync(mask, b1 ? r0 : r1, 2);  // lane%4 = 0,2,1,3 holds sum 0,1,2,3
+        for (int d = 4; d < lanes; d <<= 1) s += __shfl_xor_sync(mask, s, d);
+        if (lane < 4u) {
+            const int q = (int)((lane & 1u) * 2u + (lane >> 1));
+            if (mode == kMomDirect) mom[4 * cell + q] = s;
+            else atomicAdd(mom + 4 * cell + q, s);
+        }
+        return;
+    }
+    for (int d = 1; d < lanes; d <<= 1) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) ps[q] += __shfl_xor_sync(mask, ps[q], d);
+    }
+    if (lane == 0u) {
+        if (mode == kMomDirect) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) mom[4 * cell + q] = ps[q];
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) atomicAdd(mom + 4 * cell + q, ps[q]);
+        }
+    }
+}
+
 // Particle g = cell * ppc + j (cell-major).  A 128-bit group of G particles that lies inside one cell -- every
 // group when ppc is a multiple of G -- loads that cell's Coef<T> once and runs the same packed / shared-head
 // code as the uniform sampler; a group that straddles a cell boundary takes the per-particle path.
-template <typename T, bool VEC>
+// STORE: write the velocity planes.  MOM: also reduce (sum vx, sum vy, sum vz, sum |v|^2) per cell into
+// mom[ncell][4] -- the loader fused with its first consumer: with STORE = false
+// no velocity ever reaches HBM.
+template <typename T, bool VEC, bool STORE, bool MOM>
 __global__ void __launch_bounds__(kThreads)
 sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, const __grid_constant__ PhiloxKeys K,
                     const Coef<T>* __restrict__ W, const T* __restrict__ drift, int64_t drift_stride,
-                    T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+                    T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz, T* __restrict__ mom, int mom_mode,
+                    int mom_lanes) {
     constexpr int G = 16 / sizeof(T);
     constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
@@ -240,6 +297,17 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                             oz[e] += dz;
                         }
                     }
+                    if (MOM) {
+                        T ps[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll
+                        for (int e = 0; e < G; ++e) {
+                            ps[0] += ox[e];
+                            ps[1] += oy[e];
+                            ps[2] += oz[e];
+                            ps[3] = fma(ox[e], ox[e], fma(oy[e], oy[e], fma(oz[e], oz[e], ps[3])));
+                        }
+                        moments_out(ps, cell0, mom_mode, mom_lanes, mom);
+                    }
                 } else {
 #pragma unroll
                     for (int e = 0; e < G; ++e) {
@@ -250,9 +318,13 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                         particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
                         velocity<false>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
                         if (drift != nullptr) add_drift(drift + 3 * cell * drift_stride, ox[e], oy[e], oz[e]);
+                        if (MOM && i + e < n) {                       // only reached in kMomAtomic mode
+                            T ps[4] = {ox[e], oy[e], oz[e], fma(ox[e], ox[e], fma(oy[e], oy[e], oz[e] * oz[e]))};
+                            moments_out(ps, cell, kMomAtomic, 1, mom);
+                        }
                     }
                 }
-                store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+                if (STORE) store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
             }
         }
     }

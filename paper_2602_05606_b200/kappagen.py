@@ -44,6 +44,7 @@ def lib() -> ctypes.CDLL:
         ci = ctypes.c_int
         L.kappagen_sample.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp]
         L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
+        L.kappagen_sample_cells_moments.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, vp, sz, vp]
         L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
         L.kappagen_cells_workspace_bytes.restype = sz
         L.kappagen_sample_host.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp]
@@ -53,7 +54,7 @@ def lib() -> ctypes.CDLL:
         dp = ctypes.POINTER(ctypes.c_double)
         L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
         L.kappagen_last_error.restype = ctypes.c_char_p
-        for name in ("kappagen_sample", "kappagen_sample_cells", "kappagen_sample_host", "kappagen_baseline_mt",
+        for name in ("kappagen_sample", "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version"):
             getattr(L, name).restype = ci
         _lib = L
@@ -140,6 +141,30 @@ def sample_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None,
                                        code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), workspace.data_ptr(),
                                        workspace.numel() * workspace.element_size(), _stream(stream)))
     return vx, vy, vz
+
+
+def sample_cells_moments(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0,
+                         seed: int = 0, offset: int = 0, out=None, moments=None, workspace=None, stream=None,
+                         store: bool = True):
+    """kappagen_sample_cells_moments: returns ((vx, vy, vz) or None, moments[ncell, 4]).  store=False passes
+    NULL planes: moments only, no velocity reaches HBM."""
+    code = _dtype_code(kappa.dtype)
+    ncell = kappa.numel()
+    if theta.dtype != kappa.dtype or theta.numel() != ncell or (drift is not None and drift.dtype != kappa.dtype):
+        raise ValueError("kappa, theta and drift must share dtype; kappa and theta must share length")
+    planes = _planes(ncell * ppc, code, out, kappa.device) if store else None
+    if moments is None:
+        moments = torch.empty((ncell, 4), dtype=kappa.dtype, device=kappa.device)
+    need = cells_workspace_bytes(ncell, code)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    ptrs = [p.data_ptr() for p in planes] if store else [None, None, None]
+    _check(lib().kappagen_sample_cells_moments(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
+                                               drift.data_ptr() if drift is not None else None, drift_stride, seed,
+                                               offset, code, ptrs[0], ptrs[1], ptrs[2], moments.data_ptr(),
+                                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                               _stream(stream)))
+    return planes, moments
 
 
 def sample_host(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", out=None,
