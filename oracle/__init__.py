@@ -67,6 +67,12 @@ def lib() -> ctypes.CDLL:
             L.oracle_sample_cells.restype = ctypes.c_int
             L.oracle_cells_moments.argtypes = [i64, i32, _f64p, _f64p, _f64p, i64, u64, u64, _f64p, _f64p]
             L.oracle_cells_moments.restype = ctypes.c_int
+            L.oracle_x_of_w0w3.argtypes = [i64, _u32p, _u32p, f64, _f64p]
+            L.oracle_x_of_w0w3.restype = ctypes.c_int
+            L.oracle_sample_u64.argtypes = [i64, f64, f64, u64, u64, _f64p, _f64p, _f64p, _u32p]
+            L.oracle_sample_u64.restype = ctypes.c_int
+            L.oracle_velocity_of_words_u64.argtypes = [i64, _u32p, _u32p, _u32p, _u32p, f64, f64, _f64p, _f64p, _f64p]
+            L.oracle_velocity_of_words_u64.restype = ctypes.c_int
             L.oracle_version.restype = ctypes.c_int
             _lib = L
     return _lib
@@ -190,3 +196,29 @@ def cells_moments(ppc: int, kappa, theta, drift, drift_stride: int, seed: int, o
     if rc != 0:
         raise ValueError("bad arguments")
     return mom, abs1
+
+
+# ---- 64-bit U1 from (w0, w3): SURVEY.md section 8(f) f2, reading R20
+def x_of_w0w3(w0, w3, kappa: float) -> np.ndarray:
+    w0, w3 = _u32(w0), _u32(w3)
+    x = np.empty(w0.size, dtype=np.float64)
+    if lib().oracle_x_of_w0w3(w0.size, _p32(w0), _p32(w3), kappa, _p64(x)) != 0:
+        raise ValueError("bad kappa")
+    return x
+
+
+def sample_u64(n: int, kappa: float, theta: float, seed: int, offset: int = 0, return_w3: bool = False):
+    v = [np.empty(n, dtype=np.float64) for _ in range(3)]
+    w3 = np.empty(n, dtype=np.uint32)
+    if lib().oracle_sample_u64(n, kappa, theta, seed, offset, _p64(v[0]), _p64(v[1]), _p64(v[2]), _p32(w3)) != 0:
+        raise ValueError("bad arguments")
+    return (tuple(v), w3) if return_w3 else tuple(v)
+
+
+def velocity_of_words_u64(w0, w1, w2, w3, kappa: float, theta: float):
+    w0, w1, w2, w3 = _u32(w0), _u32(w1), _u32(w2), _u32(w3)
+    v = [np.empty(w0.size, dtype=np.float64) for _ in range(3)]
+    if lib().oracle_velocity_of_words_u64(w0.size, _p32(w0), _p32(w1), _p32(w2), _p32(w3), kappa, theta,
+                                          _p64(v[0]), _p64(v[1]), _p64(v[2])) != 0:
+        raise ValueError("bad arguments")
+    return tuple(v)

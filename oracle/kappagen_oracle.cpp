@@ -116,23 +116,41 @@ ld x_literal(uint32_t w0, const Params& P) {
 
 // ---------------------------------------------------------------- S2-S4: speed, cancellation-free
 // Same steps; each written so that nothing cancels (readings R3, R7).
-ld L_stable(uint32_t w0, const Params& P) {
-    const ld U1 = ((ld)w0 + 0.5L) / TWO32;
-    const ld t1 = ((ld)(uint32_t)(~w0) + 0.5L) / TWO32;                  // 1 - U1, exact (PAPER.md:250)
-    const ld lnU1 = (w0 < 0x80000000u) ? logl(U1) : log1pl(-t1);
+ld L_of_uniform(ld U1, ld t1, bool upper_half, const Params& P) {
+    const ld lnU1 = upper_half ? log1pl(-t1) : logl(U1);
     const ld E = (2.0L / 3.0L) * lnU1;                                    // ln U1^{2/3} <= 0
     const ld lnS = (E > -LN2_L) ? logl(-expm1l(E)) : log1pl(-expl(E));   // ln(1 - U1^{2/3})
     const ld M = -lnS / P.kstar;                                          // >= 0
     return -P.kstar * expm1l(M);                                          // Eq. (25); L < 0
 }
 
-ld x_stable(uint32_t w0, const Params& P) {
-    const ld L = L_stable(w0, P);
+ld L_stable(uint32_t w0, const Params& P) {
+    const ld U1 = ((ld)w0 + 0.5L) / TWO32;
+    const ld t1 = ((ld)(uint32_t)(~w0) + 0.5L) / TWO32;                  // 1 - U1, exact (PAPER.md:250)
+    return L_of_uniform(U1, t1, w0 >= 0x80000000u, P);
+}
+
+ld x_of_L(ld L, const Params& P) {
     const ld A = P.a + P.c * L;
     const ld D = sqrtl(A * A - 4.0L * P.b * L);                           // -4bL > 0 so D > |A|
     // Eq. (24) prints both forms of the positive root; use the one that adds.
     return (A >= 0.0L) ? (-2.0L * L / (A + D)) : ((D - A) / (2.0L * P.b));
 }
+
+ld x_stable(uint32_t w0, const Params& P) { return x_of_L(L_stable(w0, P), P); }
+
+// 64-bit U1 (reading R20): U1 = (W + 1/2)/2^64 with W = w0 2^32 + w3,
+// the word the 32-bit generator discards.  1 - U1 = (~W + 1/2)/2^64 from the integer complement again.
+// W + 1/2 needs 65 bits when W >= 2^63; there the branch uses t1 (exact for the small ~W that matter), and
+// the other way round, so each branch sees its own argument to 2^-64 relative.
+ld L_stable64(uint32_t w0, uint32_t w3, const Params& P) {
+    const uint64_t W = ((uint64_t)w0 << 32) | (uint64_t)w3;
+    const ld TWO64 = TWO32 * TWO32;
+    const ld U1 = ((ld)W + 0.5L) / TWO64;
+    const ld t1 = ((ld)(~W) + 0.5L) / TWO64;
+    return L_of_uniform(U1, t1, (W >> 63) != 0, P);
+}
+ld x_stable64(uint32_t w0, uint32_t w3, const Params& P) { return x_of_L(L_stable64(w0, w3, P), P); }
 
 // ---------------------------------------------------------------- S5: direction
 struct Dir {
@@ -224,6 +242,14 @@ int oracle_L_of_w0(int64_t n, const uint32_t* w0, double kappa, double* L) {
     return 0;
 }
 
+// The same with the 64-bit U1 built from (w0, w3).
+int oracle_x_of_w0w3(int64_t n, const uint32_t* w0, const uint32_t* w3, double kappa, double* x) {
+    if (!params_ok(kappa, 1.0)) return -1;
+    const Params P = params_of((ld)kappa);
+    for (int64_t i = 0; i < n; ++i) x[i] = (double)x_stable64(w0[i], w3[i], P);
+    return 0;
+}
+
 // Direction cosines (mu, sth*cos phi, sth*sin phi) from words (w1, w2), stable form (S5).
 void oracle_direction(int64_t n, const uint32_t* w1, const uint32_t* w2, double* nx, double* ny, double* nz) {
     for (int64_t i = 0; i < n; ++i) {
@@ -257,6 +283,37 @@ int oracle_sample(int64_t n, double kappa, double theta, uint64_t seed, uint64_t
         particle_words(seed, offset + (uint64_t)i, w);
         const ld V = (ld)theta * sqrtl(x_stable(w[0], P));
         const Dir d = dir_stable(w[1], w[2]);
+        vx[i] = (double)(V * d.mu);
+        vy[i] = (double)(V * d.sth * d.cphi);
+        vz[i] = (double)(V * d.sth * d.sphi);
+    }
+    return 0;
+}
+
+// The generator with the 64-bit U1 (flag KAPPAGEN_U1_64 of the library); w3[] (optional) receives the fourth word.
+int oracle_sample_u64(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                      double* vx, double* vy, double* vz, uint32_t* w3_out) {
+    if (n < 0 || !params_ok(kappa, theta)) return -1;
+    const Params P = params_of((ld)kappa);
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t w[4];
+        particle_words(seed, offset + (uint64_t)i, w);
+        const ld V = (ld)theta * sqrtl(x_stable64(w[0], w[3], P));
+        const Dir d = dir_stable(w[1], w[2]);
+        vx[i] = (double)(V * d.mu);
+        vy[i] = (double)(V * d.sth * d.cphi);
+        vz[i] = (double)(V * d.sth * d.sphi);
+        if (w3_out) w3_out[i] = w[3];
+    }
+    return 0;
+}
+int oracle_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2, const uint32_t* w3,
+                                 double kappa, double theta, double* vx, double* vy, double* vz) {
+    if (!params_ok(kappa, theta)) return -1;
+    const Params P = params_of((ld)kappa);
+    for (int64_t i = 0; i < n; ++i) {
+        const ld V = (ld)theta * sqrtl(x_stable64(w0[i], w3[i], P));
+        const Dir d = dir_stable(w1[i], w2[i]);
         vx[i] = (double)(V * d.mu);
         vy[i] = (double)(V * d.sth * d.cphi);
         vz[i] = (double)(V * d.sth * d.sphi);
