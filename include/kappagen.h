@@ -53,6 +53,18 @@ typedef enum {
 int kappagen_sample(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
                     int dtype, void* vx, void* vy, void* vz, void* stream);
 
+/* kappagen_sample with options.  flags = 0 is kappagen_sample.
+ *  KAPPAGEN_U1_64: U1 takes 64 bits, U1 = (w0 2^32 + w3 + 1/2)/2^64, from the first and the otherwise
+ *  discarded fourth word of the particle's Philox block (reading R20).  The paper fixes neither
+ *  the generator nor its width ("generate U1 ~ Uniform(0,1)", Table I line 5); with 32 bits
+ *  the largest speed is x_max = G^-1(1 - 2^-33) -- v/theta = 5.0e4 at kappa = 1.6, where the tail beyond
+ *  carries 12 % of <v^2> -- and 64 bits move it to G^-1(1 - 2^-65), 2^(32/kappa*) further in v^2, at no
+ *  extra random-number cost.  U2, U3 and the Philox stream are unchanged; a different (finer) generator,
+ *  not bit-compatible with flags = 0.  Unknown flag bits: KAPPAGEN_EINVAL. */
+enum { KAPPAGEN_U1_64 = 1 };
+int kappagen_sample_flags(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                          int dtype, uint32_t flags, void* vx, void* vy, void* vz, void* stream);
+
 /* Same generator with PIC-style per-cell parameters ("10^2-10^3 particles in a grid cell",
  * PAPER.md:215).  Cell-major: particle g = cell*ppc + j (0 <= j < ppc) uses counter offset + g,
  * kappa[cell], theta[cell]; the cell's drift velocity is added last, in the output type.
@@ -111,11 +123,20 @@ int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint64_t seed, u
 int kappagen_words(int64_t n, uint64_t seed, uint64_t offset,
                    uint32_t* w0, uint32_t* w1, uint32_t* w2, void* stream);
 
+/* As kappagen_words, plus the fourth word (consumed only under KAPPAGEN_U1_64).  w3: device, [n] uint32. */
+int kappagen_words4(int64_t n, uint64_t seed, uint64_t offset,
+                    uint32_t* w0, uint32_t* w1, uint32_t* w2, uint32_t* w3, void* stream);
+
 /* Test hook: velocities from caller-chosen words instead of Philox (same device math as
  * kappagen_sample, S2-S6), so parity can be driven through the extreme words.  w0,w1,w2: device. */
 int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
                                double kappa, double theta, int dtype,
                                void* vx, void* vy, void* vz, void* stream);
+
+/* As kappagen_velocity_of_words under KAPPAGEN_U1_64: U1 from (w0, w3). */
+int kappagen_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                   const uint32_t* w3, double kappa, double theta, int dtype,
+                                   void* vx, void* vy, void* vz, void* stream);
 
 /* Table I lines 1-4 on the host in double, exactly as kappagen_sample computes them before launch.
  * All four outputs are host pointers and required. */

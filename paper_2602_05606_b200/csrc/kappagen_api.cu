@@ -62,36 +62,45 @@ static int check_planes(const char* fn, int64_t n, int dtype, const void* vx, co
     return KAPPAGEN_OK;
 }
 
-template <typename T, bool VEC, bool FOLD>
+template <typename T, bool VEC, bool FOLD, bool U64>
 static int launch_sample_as(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T* vx, T* vy, T* vz,
                             cudaStream_t st) {
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * TileTraits<T>::groups;
     int grid = 0, rc;
-    if ((rc = grid_for(sample_kernel<T, VEC, FOLD>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
-    sample_kernel<T, VEC, FOLD><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
+    if ((rc = grid_for(sample_kernel<T, VEC, FOLD, U64>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
+    sample_kernel<T, VEC, FOLD, U64><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
 }
 
-static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec,
+template <typename T, bool U64>
+static int launch_sample_u(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, bool vec, bool fold, T* vx, T* vy,
+                           T* vz, cudaStream_t st) {
+    if (vec) return fold ? launch_sample_as<T, true, true, U64>(n, offset, K, C, vx, vy, vz, st)
+                         : launch_sample_as<T, true, false, U64>(n, offset, K, C, vx, vy, vz, st);
+    return fold ? launch_sample_as<T, false, true, U64>(n, offset, K, C, vx, vy, vz, st)
+                : launch_sample_as<T, false, false, U64>(n, offset, K, C, vx, vy, vz, st);
+}
+
+static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec, bool u64,
                          float* vx, float* vy, float* vz, cudaStream_t st) {
     const bool fold = theta_folds(theta);
     const Coef<float> C = host_coef_f32(kappa, theta, fold);
-    if (vec) return fold ? launch_sample_as<float, true, true>(n, offset, K, C, vx, vy, vz, st)
-                         : launch_sample_as<float, true, false>(n, offset, K, C, vx, vy, vz, st);
-    return fold ? launch_sample_as<float, false, true>(n, offset, K, C, vx, vy, vz, st)
-                : launch_sample_as<float, false, false>(n, offset, K, C, vx, vy, vz, st);
+    return u64 ? launch_sample_u<float, true>(n, offset, K, C, vec, fold, vx, vy, vz, st)
+               : launch_sample_u<float, false>(n, offset, K, C, vec, fold, vx, vy, vz, st);
 }
 
-static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec,
+static int launch_sample(int64_t n, uint64_t offset, const PhiloxKeys& K, double kappa, double theta, bool vec, bool u64,
                          double* vx, double* vy, double* vz, cudaStream_t st) {
-    const Coef<double> C = host_coef_f64(kappa, theta);
-    return vec ? launch_sample_as<double, true, false>(n, offset, K, C, vx, vy, vz, st)
-               : launch_sample_as<double, false, false>(n, offset, K, C, vx, vy, vz, st);
+    const Coef<double> C = host_coef_f64(kappa, theta);           // FOLD is a float-only notion: always false here
+    if (u64) return vec ? launch_sample_as<double, true, false, true>(n, offset, K, C, vx, vy, vz, st)
+                        : launch_sample_as<double, false, false, true>(n, offset, K, C, vx, vy, vz, st);
+    return vec ? launch_sample_as<double, true, false, false>(n, offset, K, C, vx, vy, vz, st)
+               : launch_sample_as<double, false, false, false>(n, offset, K, C, vx, vy, vz, st);
 }
 
 static int sample_on_stream(const char* fn, int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
-                            int dtype, void* vx, void* vy, void* vz, cudaStream_t st) {
+                            int dtype, uint32_t flags, void* vx, void* vy, void* vz, cudaStream_t st) {
     bool vec = false;
     int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
     if (rc != KAPPAGEN_OK) return rc;
@@ -99,10 +108,15 @@ static int sample_on_stream(const char* fn, int64_t n, double kappa, double thet
         set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
         return KAPPAGEN_EINVAL;
     }
+    if (flags & ~(uint32_t)KAPPAGEN_U1_64) {
+        set_error("%s: unknown flag bits 0x%x", fn, flags);
+        return KAPPAGEN_EINVAL;
+    }
     if (n == 0) return KAPPAGEN_OK;
     const PhiloxKeys K = philox_expand_keys(seed);
-    if (dtype == KAPPAGEN_F32) return launch_sample(n, offset, K, kappa, theta, vec, (float*)vx, (float*)vy, (float*)vz, st);
-    return launch_sample(n, offset, K, kappa, theta, vec, (double*)vx, (double*)vy, (double*)vz, st);
+    const bool u64 = (flags & KAPPAGEN_U1_64) != 0;
+    if (dtype == KAPPAGEN_F32) return launch_sample(n, offset, K, kappa, theta, vec, u64, (float*)vx, (float*)vy, (float*)vz, st);
+    return launch_sample(n, offset, K, kappa, theta, vec, u64, (double*)vx, (double*)vy, (double*)vz, st);
 }
 
 template <typename T, bool VEC, bool STORE, bool MOM>
@@ -167,7 +181,13 @@ using namespace kappagen;
 
 extern "C" int kappagen_sample(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
                                void* vx, void* vy, void* vz, void* stream) {
-    return sample_on_stream("kappagen_sample", n, kappa, theta, seed, offset, dtype, vx, vy, vz, (cudaStream_t)stream);
+    return sample_on_stream("kappagen_sample", n, kappa, theta, seed, offset, dtype, 0u, vx, vy, vz, (cudaStream_t)stream);
+}
+
+extern "C" int kappagen_sample_flags(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                                     uint32_t flags, void* vx, void* vy, void* vz, void* stream) {
+    return sample_on_stream("kappagen_sample_flags", n, kappa, theta, seed, offset, dtype, flags, vx, vy, vz,
+                            (cudaStream_t)stream);
 }
 
 extern "C" size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype) {
@@ -268,33 +288,42 @@ extern "C" int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint6
     return launch_mt<double>(n, kappa, theta, offset, K, (double*)vx, (double*)vy, (double*)vz, trip_counters, st);
 }
 
-extern "C" int kappagen_words(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
-                              void* stream) {
-    const char* fn = "kappagen_words";
+static int words_impl(const char* fn, int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
+                      uint32_t* w3, bool want_w3, void* stream) {
     if (n < 0) {
         set_error("%s: negative count", fn);
         return KAPPAGEN_EINVAL;
     }
     if (n == 0) return KAPPAGEN_OK;
-    if (!w0 || !w1 || !w2) {
+    if (!w0 || !w1 || !w2 || (want_w3 && !w3)) {
         set_error("%s: NULL output", fn);
         return KAPPAGEN_ENULL;
     }
-    if (!aligned_to(w0, 4) || !aligned_to(w1, 4) || !aligned_to(w2, 4)) {
+    if (!aligned_to(w0, 4) || !aligned_to(w1, 4) || !aligned_to(w2, 4) || !aligned_to(w3, 4)) {
         set_error("%s: outputs must be 4-byte aligned", fn);
         return KAPPAGEN_EALIGN;
     }
     int grid = 0, rc;
     if ((rc = grid_for(words_kernel, (n + 4 * kThreads - 1) / (4 * kThreads), &grid)) != KAPPAGEN_OK) return rc;
-    words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2);
+    words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2, w3);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
 }
 
-extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
-                                          double kappa, double theta, int dtype, void* vx, void* vy, void* vz,
-                                          void* stream) {
-    const char* fn = "kappagen_velocity_of_words";
+extern "C" int kappagen_words(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
+                              void* stream) {
+    return words_impl("kappagen_words", n, seed, offset, w0, w1, w2, nullptr, false, stream);
+}
+
+extern "C" int kappagen_words4(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
+                               uint32_t* w3, void* stream) {
+    return words_impl("kappagen_words4", n, seed, offset, w0, w1, w2, w3, true, stream);
+}
+
+template <bool U64>
+static int velocity_of_words_impl(const char* fn, int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                  const uint32_t* w3, double kappa, double theta, int dtype, void* vx, void* vy, void* vz,
+                                  void* stream) {
     bool vec = false;
     int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
     if (rc != KAPPAGEN_OK) return rc;
@@ -303,7 +332,7 @@ extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const u
         return KAPPAGEN_EINVAL;
     }
     if (n == 0) return KAPPAGEN_OK;
-    if (!w0 || !w1 || !w2) {
+    if (!w0 || !w1 || !w2 || (U64 && !w3)) {
         set_error("%s: NULL word array", fn);
         return KAPPAGEN_ENULL;
     }
@@ -314,19 +343,33 @@ extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const u
         const bool fold = theta_folds(theta);              // the same choice kappagen_sample makes
         const Coef<float> C = host_coef_f32(kappa, theta, fold);
         if (fold) {
-            if ((rc = grid_for(velocity_of_words_kernel<float, true>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-            velocity_of_words_kernel<float, true><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, C, (float*)vx, (float*)vy, (float*)vz);
+            if ((rc = grid_for(velocity_of_words_kernel<float, true, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            velocity_of_words_kernel<float, true, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, C, (float*)vx, (float*)vy, (float*)vz);
         } else {
-            if ((rc = grid_for(velocity_of_words_kernel<float, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-            velocity_of_words_kernel<float, false><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, C, (float*)vx, (float*)vy, (float*)vz);
+            if ((rc = grid_for(velocity_of_words_kernel<float, false, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            velocity_of_words_kernel<float, false, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, C, (float*)vx, (float*)vy, (float*)vz);
         }
     } else {
-        if ((rc = grid_for(velocity_of_words_kernel<double, false>, tiles, &grid)) != KAPPAGEN_OK) return rc;
-        velocity_of_words_kernel<double, false><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, host_coef_f64(kappa, theta),
-                                                                           (double*)vx, (double*)vy, (double*)vz);
+        if ((rc = grid_for(velocity_of_words_kernel<double, false, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        velocity_of_words_kernel<double, false, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, host_coef_f64(kappa, theta),
+                                                                                (double*)vx, (double*)vy, (double*)vz);
     }
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_velocity_of_words(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                          double kappa, double theta, int dtype, void* vx, void* vy, void* vz,
+                                          void* stream) {
+    return velocity_of_words_impl<false>("kappagen_velocity_of_words", n, w0, w1, w2, nullptr, kappa, theta, dtype, vx, vy, vz,
+                                         stream);
+}
+
+extern "C" int kappagen_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                              const uint32_t* w3, double kappa, double theta, int dtype, void* vx, void* vy,
+                                              void* vz, void* stream) {
+    return velocity_of_words_impl<true>("kappagen_velocity_of_words_u64", n, w0, w1, w2, w3, kappa, theta, dtype, vx, vy, vz,
+                                        stream);
 }
 
 // End-to-end path: host destination, chunked, double-buffered (the copy of chunk c overlaps the kernel
@@ -359,7 +402,7 @@ extern "C" int kappagen_sample_host(int64_t n, double kappa, double theta, uint6
         const int b = c & 1;
         const int64_t m = (n - done) < chunk ? (n - done) : chunk;
         char* d = dev + (size_t)b * 3 * plane;
-        status = sample_on_stream(fn, m, kappa, theta, seed, offset + (uint64_t)done, dtype, d, d + plane, d + 2 * plane, st[b]);
+        status = sample_on_stream(fn, m, kappa, theta, seed, offset + (uint64_t)done, dtype, 0u, d, d + plane, d + 2 * plane, st[b]);
         if (status != KAPPAGEN_OK) break;
         char* hv[3] = {(char*)vx_host, (char*)vy_host, (char*)vz_host};
         for (int q = 0; q < 3; ++q) {

@@ -43,55 +43,57 @@ template <typename T> struct Vec128;
 template <> struct Vec128<float> { using type = float4; };
 template <> struct Vec128<double> { using type = double2; };
 
-// FOLD (float only): theta is folded into the coefficients, see coefs.cuh.
-template <bool FOLD>
-__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<float>& C,
-                                         float& x, float& y, float& z) { velocity_f32<FOLD>(w0, w1, w2, C, x, y, z); }
-template <bool FOLD>
-__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, const Coef<double>& C,
-                                         double& x, double& y, double& z) { velocity_f64(w0, w1, w2, C, x, y, z); }
+// FOLD (float only): theta is folded into the coefficients, see coefs.cuh.  U64: U1 takes 64 bits from
+// (w0, w3) instead of 32 from w0 (reading R20); w3 is ignored otherwise.
+template <bool FOLD, bool U64 = false>
+__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, const Coef<float>& C,
+                                         float& x, float& y, float& z) { velocity_f32<FOLD, U64>(w0, w1, w2, w3, C, x, y, z); }
+template <bool FOLD, bool U64 = false>
+__device__ __forceinline__ void velocity(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, const Coef<double>& C,
+                                         double& x, double& y, double& z) { velocity_f64<U64>(w0, w1, w2, w3, C, x, y, z); }
 
 // The Philox words of G consecutive particles starting at global counter g0.  Unless the low counter
 // word wraps inside the group (one group in 2^32 particles; a uniform branch everywhere else) the
 // particles share hi32(g) and with it the head of the Philox block (philox.cuh).
 template <int G>
 __device__ __forceinline__ void group_words(uint64_t g0, const PhiloxKeys& K, uint32_t (&w0)[G], uint32_t (&w1)[G],
-                                            uint32_t (&w2)[G]) {
+                                            uint32_t (&w2)[G], uint32_t (&w3)[G]) {
     const uint32_t lo = (uint32_t)g0, hi = (uint32_t)(g0 >> 32);
     if (lo <= 0xFFFFFFFFu - (uint32_t)(G - 1)) {
         const PhiloxHead H = philox_head(hi, K);
 #pragma unroll
-        for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e]);
+        for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
     } else {
 #pragma unroll
-        for (int e = 0; e < G; ++e) particle_words(g0 + (uint64_t)e, K, w0[e], w1[e], w2[e]);
+        for (int e = 0; e < G; ++e) particle_words(g0 + (uint64_t)e, K, w0[e], w1[e], w2[e], w3[e]);
     }
 }
 
 // One 128-bit group: G consecutive particles starting at global counter g0.  float: two packed pairs
 // (math_f32x2.cuh, bit-identical to the scalar chain); double: two scalar chains.
-template <bool FOLD>
+template <bool FOLD, bool U64 = false>
 __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<float>& C,
                                                  float (&ox)[4], float (&oy)[4], float (&oz)[4]) {
-    uint32_t w0[4], w1[4], w2[4];
-    group_words<4>(g0, K, w0, w1, w2);
+    uint32_t w0[4], w1[4], w2[4], w3[4];
+    group_words<4>(g0, K, w0, w1, w2, w3);
 #pragma unroll
     for (int e = 0; e < 4; e += 2) {
         const uint32_t p0[2] = {w0[e], w0[e + 1]}, p1[2] = {w1[e], w1[e + 1]}, p2[2] = {w2[e], w2[e + 1]};
+        const uint32_t p3[2] = {w3[e], w3[e + 1]};
         float a[2], b[2], c[2];
-        velocity_pair_f32<FOLD>(p0, p1, p2, C, a, b, c);
+        velocity_pair_f32<FOLD, U64>(p0, p1, p2, p3, C, a, b, c);
         ox[e] = a[0]; ox[e + 1] = a[1];
         oy[e] = b[0]; oy[e + 1] = b[1];
         oz[e] = c[0]; oz[e + 1] = c[1];
     }
 }
-template <bool FOLD>
+template <bool FOLD, bool U64 = false>
 __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<double>& C,
                                                  double (&ox)[2], double (&oy)[2], double (&oz)[2]) {
-    uint32_t w0[2], w1[2], w2[2];
-    group_words<2>(g0, K, w0, w1, w2);
+    uint32_t w0[2], w1[2], w2[2], w3[2];
+    group_words<2>(g0, K, w0, w1, w2, w3);
 #pragma unroll
-    for (int e = 0; e < 2; ++e) velocity_f64(w0[e], w1[e], w2[e], C, ox[e], oy[e], oz[e]);
+    for (int e = 0; e < 2; ++e) velocity_f64<U64>(w0[e], w1[e], w2[e], w3[e], C, ox[e], oy[e], oz[e]);
 }
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
@@ -123,19 +125,19 @@ __device__ __forceinline__ void store_planes(int64_t i, int64_t n, T* __restrict
 
 // ---------------------------------------------------------------- kappagen_sample
 // Group j of the tile at `base`, bounds-checked (ragged tail, unaligned planes).
-template <typename T, bool VEC, bool FOLD>
+template <typename T, bool VEC, bool FOLD, bool U64>
 __device__ __forceinline__ void tile_group(int64_t base, int j, int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C,
                                            T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     constexpr int G = 16 / sizeof(T);
     const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
     if (i < n) {
         T ox[G], oy[G], oz[G];
-        group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox, oy, oz);
+        group_velocities<FOLD, U64>(offset + (uint64_t)i, K, C, ox, oy, oz);
         store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
     }
 }
 
-template <typename T, bool VEC, bool FOLD>
+template <typename T, bool VEC, bool FOLD, bool U64>
 __global__ void __launch_bounds__(kThreads, TileTraits<T>::minb)
 sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
               T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
@@ -150,7 +152,7 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
                 const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
-                group_velocities<FOLD>(offset + (uint64_t)i, K, C, ox[j], oy[j], oz[j]);
+                group_velocities<FOLD, U64>(offset + (uint64_t)i, K, C, ox[j], oy[j], oz[j]);
             }
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
@@ -163,10 +165,10 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
         }
         if constexpr (TileTraits<T>::joint) {
 #pragma unroll 1
-            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD>(base, j, n, offset, K, C, vx, vy, vz);
+            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD, U64>(base, j, n, offset, K, C, vx, vy, vz);
         } else {
 #pragma unroll
-            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD>(base, j, n, offset, K, C, vx, vy, vz);
+            for (int j = 0; j < NG; ++j) tile_group<T, VEC, FOLD, U64>(base, j, n, offset, K, C, vx, vy, vz);
         }
     }
 }
@@ -316,7 +318,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                         const Coef<T> C = W[cell];
                         uint32_t w0, w1, w2;
                         particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                        velocity<false>(w0, w1, w2, C, ox[e], oy[e], oz[e]);
+                        velocity<false>(w0, w1, w2, 0u, C, ox[e], oy[e], oz[e]);
                         if (drift != nullptr) add_drift(drift + 3 * cell * drift_stride, ox[e], oy[e], oz[e]);
                         if (MOM && i + e < n) {                       // only reached in kMomAtomic mode
                             T ps[4] = {ox[e], oy[e], oz[e], fma(ox[e], ox[e], fma(oy[e], oy[e], oz[e] * oz[e]))};
@@ -333,30 +335,31 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
 // ---------------------------------------------------------------- test hooks
 __global__ void __launch_bounds__(kThreads)
 words_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,
-             uint32_t* __restrict__ o1, uint32_t* __restrict__ o2) {
+             uint32_t* __restrict__ o1, uint32_t* __restrict__ o2, uint32_t* __restrict__ o3) {
     // four consecutive particles per thread through group_words, exactly as the fp32 sampler draws them
     for (int64_t i = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4; i < n; i += (int64_t)gridDim.x * kThreads * 4) {
-        uint32_t w0[4], w1[4], w2[4];
-        group_words<4>(offset + (uint64_t)i, K, w0, w1, w2);
+        uint32_t w0[4], w1[4], w2[4], w3[4];
+        group_words<4>(offset + (uint64_t)i, K, w0, w1, w2, w3);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             if (i + e < n) {
                 o0[i + e] = w0[e];
                 o1[i + e] = w1[e];
                 o2[i + e] = w2[e];
+                if (o3 != nullptr) o3[i + e] = w3[e];
             }
         }
     }
 }
 
-template <typename T, bool FOLD>
+template <typename T, bool FOLD, bool U64>
 __global__ void __launch_bounds__(kThreads)
 velocity_of_words_kernel(int64_t n, const uint32_t* __restrict__ w0, const uint32_t* __restrict__ w1,
-                         const uint32_t* __restrict__ w2, const __grid_constant__ Coef<T> C,
+                         const uint32_t* __restrict__ w2, const uint32_t* __restrict__ w3, const __grid_constant__ Coef<T> C,
                          T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
         T x, y, z;
-        velocity<FOLD>(w0[i], w1[i], w2[i], C, x, y, z);
+        velocity<FOLD, U64>(w0[i], w1[i], w2[i], U64 ? w3[i] : 0u, C, x, y, z);
         vx[i] = x;
         vy[i] = y;
         vz[i] = z;

@@ -31,12 +31,27 @@ __device__ __forceinline__ float mufu_rcp(float x) { float y; asm("rcp.approx.ft
 __device__ __forceinline__ float mufu_rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float mufu_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+// 2^32 U1 and 1 - U1 as floats with RELATIVE accuracy at both ends.  U64 (reading R20): U1 = (w0 2^32 + w3 +
+// 1/2)/2^64; the low word only matters where the high word (or its complement) is small.
+template <bool U64>
+__device__ __forceinline__ void uniform1_f32(uint32_t w0, uint32_t w3, float& u_scaled, float& t1) {
+    if (U64) {
+        u_scaled = (float)w0 + fmaf((float)w3, 0x1p-32f, 0x1p-33f);
+        t1 = fmaf((float)(uint32_t)(~w0), 0x1p-32f, fmaf((float)(uint32_t)(~w3), 0x1p-64f, 0x1p-65f));
+    } else {
+        u_scaled = (float)w0 + 0.5f;
+        t1 = fmaf((float)(uint32_t)(~w0), 0x1p-32f, 0x1p-33f);               // 1 - U1 from the integer
+    }
+}
+
 // 2V = 2 theta sqrt(x) (times 1/theta when the coefficients are not folded, see Coef<float>).
-__device__ __forceinline__ float speed2_f32(uint32_t w0, const Coef<float>& C) {
-    // r = U1^(1/3) = 2^((log2(w0 + 1/2) - 32)/3); only p = r^2 small needs it to relative accuracy
-    const float lg = mufu_lg2((float)w0 + 0.5f);
+template <bool U64 = false>
+__device__ __forceinline__ float speed2_f32(uint32_t w0, uint32_t w3, const Coef<float>& C) {
+    // r = U1^(1/3) = 2^((log2(2^32 U1) - 32)/3); only p = r^2 small needs it to relative accuracy
+    float us, t1;
+    uniform1_f32<U64>(w0, w3, us, t1);
+    const float lg = mufu_lg2(us);
     const float r = mufu_ex2(fmaf(lg, 0x1.555556p-2f, -0x1.555556p+3f));
-    const float t1 = fmaf((float)(uint32_t)(~w0), 0x1p-32f, 0x1p-33f);      // 1 - U1 from the integer
     const float p = r * r;                                                    // U1^(2/3)
     const float q1 = r + 1.0f;
     const float S = (t1 * q1) * mufu_rcp(q1 + p);                             // 1 - U1^(2/3), no cancellation
@@ -99,10 +114,10 @@ __device__ __forceinline__ void direction_f32(uint32_t w1, uint32_t w2, float& m
 
 // FOLD: theta is already inside C.k2 / C.th4 (uniform-parameter kernels); otherwise multiply by C.theta
 // (per-cell parameters, theta = 0, or theta outside [2^-30, 2^30]).
-template <bool FOLD>
-__device__ __forceinline__ void velocity_f32(uint32_t w0, uint32_t w1, uint32_t w2,
+template <bool FOLD, bool U64 = false>
+__device__ __forceinline__ void velocity_f32(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3,
                                              const Coef<float>& C, float& vx, float& vy, float& vz) {
-    float V2 = speed2_f32(w0, C);                      // 2V
+    float V2 = speed2_f32<U64>(w0, w3, C);             // 2V
     if (!FOLD) V2 *= C.theta;
     float muh, sth, cphi, sphi;
     direction_f32(w1, w2, muh, sth, cphi, sphi);

@@ -24,10 +24,15 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f
 #define KG_MAP2(fn, v) ([&] { float a_, b_; up2((v), a_, b_); return pk2(fn(a_), fn(b_)); }())
 
 // 2V for two particles (see speed2_f32).
-__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, const Coef<float>& C) {
-    const f32x2 lg = KG_MAP2(mufu_lg2, add2(pk2((float)w0a, (float)w0b), splat2(0.5f)));
+template <bool U64>
+__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32_t w3a, uint32_t w3b, const Coef<float>& C) {
+    // 2^32 U1 and 1 - U1 (uniform1_f32, packed); U64: the fourth word refines both where the first is small
+    const f32x2 ulo = U64 ? fma2(pk2((float)w3a, (float)w3b), splat2(0x1p-32f), splat2(0x1p-33f)) : splat2(0.5f);
+    const f32x2 tlo = U64 ? fma2(pk2((float)(uint32_t)(~w3a), (float)(uint32_t)(~w3b)), splat2(0x1p-64f), splat2(0x1p-65f))
+                          : splat2(0x1p-33f);
+    const f32x2 lg = KG_MAP2(mufu_lg2, add2(pk2((float)w0a, (float)w0b), ulo));
     const f32x2 r = KG_MAP2(mufu_ex2, fma2(lg, splat2(0x1.555556p-2f), splat2(-0x1.555556p+3f)));
-    const f32x2 t1 = fma2(pk2((float)(uint32_t)(~w0a), (float)(uint32_t)(~w0b)), splat2(0x1p-32f), splat2(0x1p-33f));
+    const f32x2 t1 = fma2(pk2((float)(uint32_t)(~w0a), (float)(uint32_t)(~w0b)), splat2(0x1p-32f), tlo);
     const f32x2 p = mul2(r, r);
     const f32x2 q1 = add2(r, splat2(1.0f));
     const f32x2 S = mul2(mul2(t1, q1), KG_MAP2(mufu_rcp, add2(q1, p)));
@@ -74,10 +79,11 @@ __device__ __forceinline__ void quadrant_f32(uint32_t w2, float sr, float cr, fl
     sphi = __uint_as_float(__float_as_uint(s0) ^ (wq & 0x80000000u));
 }
 
-template <bool FOLD>
+template <bool FOLD, bool U64 = false>
 __device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
-                                                  const Coef<float>& C, float (&vx)[2], float (&vy)[2], float (&vz)[2]) {
-    f32x2 V2 = speed2_f32x2(w0[0], w0[1], C);
+                                                  const uint32_t (&w3)[2], const Coef<float>& C, float (&vx)[2],
+                                                  float (&vy)[2], float (&vz)[2]) {
+    f32x2 V2 = speed2_f32x2<U64>(w0[0], w0[1], w3[0], w3[1], C);
     if (!FOLD) V2 = mul2(V2, splat2(C.theta));
     const f32x2 muh = fma2(pk2((float)(int32_t)(w1[0] ^ 0x80000000u), (float)(int32_t)(w1[1] ^ 0x80000000u)),
                            splat2(0x1p-32f), splat2(0x1p-33f));

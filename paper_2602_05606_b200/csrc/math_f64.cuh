@@ -75,13 +75,24 @@ __device__ __forceinline__ double sqrt3_f64(double z) {
     return fma(t, q * e, t);
 }
 
-__device__ __forceinline__ double speed_f64(uint32_t w0, const Coef<double>& C) {
-    const double u1 = u32_affine(w0, 0x1p-32, -0x1p20 + 0x1p-33);               // U1 = (w0 + 1/2)/2^32, exact
-    const double t1 = 1.0 - u1;                                                  // exact: U1 has 33 significant bits
+template <bool U64 = false>
+__device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef<double>& C) {
+    double u1, t1;
+    float useed;                                                                 // 2^32 U1 for the fp32 seed
+    if (U64) {
+        // reading R20: U1 = (w0 2^32 + w3 + 1/2)/2^64 (65 bits, rounded once); 1 - U1 from the complements
+        u1 = u32_affine(w0, 0x1p-32, -0x1p20) + u32_affine(w3, 0x1p-64, -0x1p-12 + 0x1p-65);
+        t1 = u32_affine(~w0, 0x1p-32, -0x1p20) + u32_affine(~w3, 0x1p-64, -0x1p-12 + 0x1p-65);
+        useed = (float)w0 + fmaf((float)w3, 0x1p-32f, 0x1p-33f);
+    } else {
+        u1 = u32_affine(w0, 0x1p-32, -0x1p20 + 0x1p-33);                        // U1 = (w0 + 1/2)/2^32, exact
+        t1 = 1.0 - u1;                                                           // exact: U1 has 33 significant bits
+        useed = (float)w0 + 0.5f;
+    }
     // r = U1^(1/3): fp32 seed y0 ~ U1^(-1/3) = 2^((32 - log2(w0 + 1/2))/3); r0 = u y0^2, e = 1 - u y0^3 = 1 - r0 y0,
     // r = u y^2 with y = y0 (1-e)^(-1/3):  r = r0 (1 + 2e/3 + 5e^2/9), residual ~ e^3
     float lg, ys;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"((float)w0 + 0.5f));
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(useed));
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ys) : "f"(fmaf(lg, -0x1.555556p-2f, 0x1.555556p+3f)));
     const double y0 = seed_out(ys);
     const double r0 = (y0 * y0) * u1;
@@ -134,9 +145,10 @@ __device__ __forceinline__ double speed_f64(uint32_t w0, const Coef<double>& C) 
     return C.theta * (nm * rsqrt3_f64(nm * dn));
 }
 
-__device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t w2,
+template <bool U64 = false>
+__device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3,
                                              const Coef<double>& C, double& vx, double& vy, double& vz) {
-    const double V = speed_f64(w0, C);
+    const double V = speed_f64<U64>(w0, w3, C);
     const double u2 = u32_affine(w1, 0x1p-32, -0x1p20 + 0x1p-33);               // U2, exact
     const double t2 = 1.0 - u2;                                                  // 1 - U2, exact
     const double mu = u2 - t2;                                                   // 2 U2 - 1, exact

@@ -69,7 +69,7 @@ __device__ __forceinline__ PhiloxHead philox_head(uint32_t g_hi, const PhiloxKey
 }
 // Same words as particle_words(g, ...) for g = (g_hi << 32) | g_lo, given H = philox_head(g_hi, K).
 __device__ __forceinline__ void particle_words_head(uint32_t g_lo, const PhiloxHead& H, const PhiloxKeys& K,
-                                                    uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+                                                    uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3) {
     // round 1 (c2 = c3 = 0): c = (g_hi ^ k0[0], 0, hi(M0 g_lo) ^ k1[0], lo(M0 g_lo))
     const uint64_t q0 = (uint64_t)kPhiloxM0 * (uint64_t)g_lo;
     // round 2: the M0 product is the shared head; c1 = 0
@@ -89,14 +89,19 @@ __device__ __forceinline__ void particle_words_head(uint32_t g_lo, const PhiloxH
         c0 = n0;
         c2 = n2;
     }
-    w0 = c0; w1 = c1; w2 = c2;
+    w0 = c0; w1 = c1; w2 = c2; w3 = c3;
 }
 
-// The three words particle g consumes (w3 is drawn and discarded, reading R4).
+// The words of particle g.  The samplers consume w0, w1, w2; w3 is drawn and discarded (DESIGN.md reading
+// R4) unless the caller asks for the 64-bit U1 (reading R20), and is dead code when unused.
+__device__ __forceinline__ void particle_words(uint64_t g, const PhiloxKeys& K, uint32_t& w0,
+                                               uint32_t& w1, uint32_t& w2, uint32_t& w3) {
+    philox4x32_10((uint32_t)g, (uint32_t)(g >> 32), 0u, 0u, K, w0, w1, w2, w3);
+}
 __device__ __forceinline__ void particle_words(uint64_t g, const PhiloxKeys& K, uint32_t& w0,
                                                uint32_t& w1, uint32_t& w2) {
     uint32_t w3;
-    philox4x32_10((uint32_t)g, (uint32_t)(g >> 32), 0u, 0u, K, w0, w1, w2, w3);
+    particle_words(g, K, w0, w1, w2, w3);
     (void)w3;
 }
 #endif  // __CUDACC__

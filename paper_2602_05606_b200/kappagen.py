@@ -14,6 +14,7 @@ import os
 import torch
 
 F32, F64 = 0, 1
+U1_64 = 1                      # kappagen_sample_flags: 64-bit U1 from (w0, w3)
 OK, EINVAL, ENULL, EALIGN, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4, -5
 _STATUS = {EINVAL: "KAPPAGEN_EINVAL", ENULL: "KAPPAGEN_ENULL", EALIGN: "KAPPAGEN_EALIGN",
            EWORKSPACE: "KAPPAGEN_EWORKSPACE", ECUDA: "KAPPAGEN_ECUDA"}
@@ -43,6 +44,9 @@ def lib() -> ctypes.CDLL:
                                       ctypes.c_void_p, ctypes.c_size_t)
         ci = ctypes.c_int
         L.kappagen_sample.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp]
+        L.kappagen_sample_flags.argtypes = [i64, f64, f64, u64, u64, ci, ctypes.c_uint32, vp, vp, vp, vp]
+        L.kappagen_words4.argtypes = [i64, u64, u64, vp, vp, vp, vp, vp]
+        L.kappagen_velocity_of_words_u64.argtypes = [i64, vp, vp, vp, vp, f64, f64, ci, vp, vp, vp, vp]
         L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
         L.kappagen_sample_cells_moments.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, vp, sz, vp]
         L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
@@ -54,7 +58,8 @@ def lib() -> ctypes.CDLL:
         dp = ctypes.POINTER(ctypes.c_double)
         L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
         L.kappagen_last_error.restype = ctypes.c_char_p
-        for name in ("kappagen_sample", "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
+        for name in ("kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
+                     "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version"):
             getattr(L, name).restype = ci
         _lib = L
@@ -118,6 +123,16 @@ def sample(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype
     vx, vy, vz = _planes(n, code, out, device)
     _check(lib().kappagen_sample(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
                                  _stream(stream)))
+    return vx, vy, vz
+
+
+def sample_flags(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", flags: int = 0, out=None,
+                 stream=None, device="cuda"):
+    """kappagen_sample_flags: kappagen_sample with options (flags = U1_64: 64-bit U1 from (w0, w3))."""
+    code = _dtype_code(dtype)
+    vx, vy, vz = _planes(n, code, out, device)
+    _check(lib().kappagen_sample_flags(n, kappa, theta, seed, offset, code, flags, vx.data_ptr(), vy.data_ptr(),
+                                       vz.data_ptr(), _stream(stream)))
     return vx, vy, vz
 
 
@@ -198,6 +213,27 @@ def words(n: int, seed: int, offset: int = 0, stream=None, device="cuda"):
     w = tuple(torch.empty(n, dtype=torch.int32, device=device) for _ in range(3))
     _check(lib().kappagen_words(n, seed, offset, w[0].data_ptr(), w[1].data_ptr(), w[2].data_ptr(), _stream(stream)))
     return w
+
+
+def words4(n: int, seed: int, offset: int = 0, stream=None, device="cuda"):
+    """kappagen_words4: all four words of each particle's Philox block (int32 tensors holding uint32 bits)."""
+    w = tuple(torch.empty(n, dtype=torch.int32, device=device) for _ in range(4))
+    _check(lib().kappagen_words4(n, seed, offset, w[0].data_ptr(), w[1].data_ptr(), w[2].data_ptr(), w[3].data_ptr(),
+                                 _stream(stream)))
+    return w
+
+
+def velocity_of_words_u64(w0, w1, w2, w3, kappa: float, theta: float, dtype="f32", stream=None):
+    """kappagen_velocity_of_words_u64: S2-S6 with the 64-bit U1 from (w0, w3)."""
+    code = _dtype_code(dtype)
+    n = w0.numel()
+    for w in (w0, w1, w2, w3):
+        if w.dtype != torch.int32 or w.numel() != n or not w.is_contiguous():
+            raise ValueError("words must be contiguous int32 tensors of equal length")
+    vx, vy, vz = _planes(n, code, None, w0.device)
+    _check(lib().kappagen_velocity_of_words_u64(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(), w3.data_ptr(), kappa,
+                                                theta, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
+    return vx, vy, vz
 
 
 def velocity_of_words(w0, w1, w2, kappa: float, theta: float, dtype="f32", stream=None):
