@@ -138,6 +138,25 @@ int kappagen_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t
                                    const uint32_t* w3, double kappa, double theta, int dtype,
                                    void* vx, void* vy, void* vz, void* stream);
 
+/* Paper test 2 on the device: generate n particles and count
+ * their speeds |v|/theta in bins of width dv ("Delta v = 1/5") WITHOUT writing a velocity: S1-S4 only, in
+ * the arithmetic of `dtype`, so 2^34 particles and more are a matter of milliseconds per 2^28.
+ *   bin(i) = min(floor((|v|/theta) / dv), nbins - 1): the last bin is open-ended (reading R21).
+ *   hist : device, [nbins] unsigned 64-bit counters, ACCUMULATED into (the caller zeroes them once and may
+ *          call repeatedly with consecutive offsets).  theta does not enter (speeds are in units of theta).
+ *   flags: 0 or KAPPAGEN_U1_64.   2 <= nbins <= 4096, dv > 0, n <= 2^40 per call. */
+int kappagen_speed_histogram(int64_t n, double kappa, uint64_t seed, uint64_t offset, int dtype, uint32_t flags,
+                             double dv, int32_t nbins, unsigned long long* hist, void* stream);
+
+/* The discrete relative entropy of Eqs. (26)-(27), of a HOST copy of such a histogram:
+ *   D(P||Q) = sum_i (P(i) + eps) ln((P(i) + eps)/(Q(i) + eps)),  Q(i) = hist[i]/N,  eps = 1e-10 in the paper,
+ * P(i) = the baseline distribution integrated over bin i: which = KAPPAGEN_ENTROPY_VS_EXACT: the Kappa
+ * distribution through its CDF Eq. (3), I_{x/(x+kappa)}(3/2, kappa-1/2); KAPPAGEN_ENTROPY_VS_APPROX: the
+ * generator's own CDF G, Eq. (7).  Host arithmetic only (long double); hist and D_out are host pointers. */
+enum { KAPPAGEN_ENTROPY_VS_EXACT = 0, KAPPAGEN_ENTROPY_VS_APPROX = 1 };
+int kappagen_relative_entropy(const unsigned long long* hist, int32_t nbins, double dv, double kappa,
+                              double eps, int which, double* D_out);
+
 /* Table I lines 1-4 on the host in double, exactly as kappagen_sample computes them before launch.
  * All four outputs are host pointers and required. */
 int kappagen_params(double kappa, double* kappa_star, double* a, double* b, double* c);

@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
             L.oracle_sample_u64.restype = ctypes.c_int
             L.oracle_velocity_of_words_u64.argtypes = [i64, _u32p, _u32p, _u32p, _u32p, f64, f64, _f64p, _f64p, _f64p]
             L.oracle_velocity_of_words_u64.restype = ctypes.c_int
+            L.oracle_speed_over_theta.argtypes = [i64, f64, u64, u64, ctypes.c_int, _f64p]
+            L.oracle_speed_over_theta.restype = ctypes.c_int
             L.oracle_version.restype = ctypes.c_int
             _lib = L
     return _lib
@@ -222,3 +224,48 @@ def velocity_of_words_u64(w0, w1, w2, w3, kappa: float, theta: float):
                                           _p64(v[0]), _p64(v[1]), _p64(v[2])) != 0:
         raise ValueError("bad arguments")
     return tuple(v)
+
+
+# ---- paper test 2: speed histogram and discrete relative entropy, SURVEY.md section 8(f) f3
+def speed_over_theta(n: int, kappa: float, seed: int, offset: int = 0, u64: bool = False) -> np.ndarray:
+    """|v|/theta = sqrt(x) per particle (S1-S4), long double rounded to double."""
+    s = np.empty(n, dtype=np.float64)
+    if lib().oracle_speed_over_theta(n, kappa, seed, offset, 1 if u64 else 0, _p64(s)) != 0:
+        raise ValueError("bad arguments")
+    return s
+
+
+def speed_histogram(s, dv: float, nbins: int) -> np.ndarray:
+    """Counts of s = |v|/theta in bins [i dv, (i+1) dv), i < nbins-1; the last bin is open-ended (reading R21)."""
+    idx = np.minimum(np.floor(np.asarray(s, dtype=np.float64) / dv).astype(np.int64), nbins - 1)
+    return np.bincount(idx, minlength=nbins).astype(np.uint64)
+
+
+def bin_probabilities(kappa: float, dv: float, nbins: int, which: str = "exact") -> np.ndarray:
+    """P(i): the distribution of |v|/theta integrated over each bin.  "exact": the Kappa distribution, Eq. (2)
+    integrated through its CDF Eq. (3), F(x) = I_{x/(x+kappa)}(3/2, kappa-1/2), x = v^2/theta^2.
+    "approx": the generator's own CDF G(x), Eq. (7)/(A11)."""
+    from scipy import special
+    v = np.arange(nbins, dtype=np.float64) * dv
+    x = v * v
+    # survival functions 1 - CDF at the lower bin edges, each formed without cancellation so that the far
+    # tail bins keep their relative accuracy: 1 - I_y(a,b) = I_{1-y}(b,a);  1 - (1-q)^{3/2} = -expm1(1.5 log1p(-q))
+    if which == "exact":
+        surv = special.betainc(kappa - 0.5, 1.5, kappa / (x + kappa))
+    else:
+        ks, a, b, c = params(kappa)
+        h = (a * x + b * x * x) / (1.0 + c * x)
+        q = np.exp(-ks * np.log1p(h / ks))                    # exp_{q*}(-h), Eq. (8)
+        with np.errstate(divide="ignore"):
+            surv = -np.expm1(1.5 * np.log1p(-q))             # q = 1 at v = 0: survival 1
+        surv[0] = 1.0
+    return -np.diff(np.concatenate([surv, [0.0]]))            # last bin open-ended
+
+
+def relative_entropy(hist, kappa: float, dv: float, eps: float = 1e-10, which: str = "exact") -> float:
+    """Eq. (27): D(P||Q) = sum_i (P(i)+eps) ln((P(i)+eps)/(Q(i)+eps)), P the baseline
+    (analytic) bin probabilities, Q(i) = hist[i]/N the Monte Carlo ones, eps = 1e-10."""
+    hist = np.asarray(hist, dtype=np.float64)
+    P = bin_probabilities(kappa, dv, hist.size, which)
+    Q = hist / hist.sum()
+    return float(np.sum((P + eps) * np.log((P + eps) / (Q + eps))))

@@ -321,6 +321,19 @@ int oracle_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t* 
     return 0;
 }
 
+// Speed over theta, sqrt(x), of each particle (S1-S4 only): the quantity paper test 2 histograms with bins
+// of width Delta v = 1/5.  u64 != 0: the 64-bit U1 of reading R20.
+int oracle_speed_over_theta(int64_t n, double kappa, uint64_t seed, uint64_t offset, int u64, double* s) {
+    if (n < 0 || !params_ok(kappa, 1.0)) return -1;
+    const Params P = params_of((ld)kappa);
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t w[4];
+        particle_words(seed, offset + (uint64_t)i, w);
+        s[i] = (double)sqrtl(u64 ? x_stable64(w[0], w[3], P) : x_stable(w[0], P));
+    }
+    return 0;
+}
+
 // Table I typed in verbatim (see header).  Same interface as oracle_sample.
 int oracle_sample_literal(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
                           double* vx, double* vy, double* vz) {

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libkappagen.so")
 CU_SOURCES = ["kappagen_api.cu"]
-CPP_SOURCES = ["host_params.cpp"]
+CPP_SOURCES = ["host_params.cpp", "host_entropy.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"]
 

@@ -1,6 +1,7 @@
 // kappagen_api.cu -- the C ABI of include/kappagen.h: argument checks and kernel launches.
 // Every step of the hot path runs in the kernels of kernels.cuh; nothing here computes a velocity,
 // and there is no CPU fallback: without a CUDA device the calls return KAPPAGEN_ECUDA.
+#include <cmath>
 #include <cstdint>
 #include <cstdio>
 #include <cuda_runtime.h>
@@ -308,6 +309,55 @@ static int words_impl(const char* fn, int64_t n, uint64_t seed, uint64_t offset,
     words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2, w3);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
+}
+
+template <typename T, bool U64>
+static int launch_hist(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T inv, int nbins,
+                       unsigned long long* hist, cudaStream_t st) {
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    int replicas = (48 * 1024) / (nbins * 4);
+    if (replicas > kThreads / 32) replicas = kThreads / 32;
+    if (replicas < 1) replicas = 1;
+    int grid = 0, rc;
+    if ((rc = grid_for(speed_histogram_kernel<T, U64>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
+    speed_histogram_kernel<T, U64><<<grid, kThreads, (size_t)replicas * nbins * 4, st>>>(n, offset, K, C, inv, nbins, replicas, hist);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_speed_histogram(int64_t n, double kappa, uint64_t seed, uint64_t offset, int dtype, uint32_t flags,
+                                        double dv, int32_t nbins, unsigned long long* hist, void* stream) {
+    const char* fn = "kappagen_speed_histogram";
+    if (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64) {
+        set_error("%s: dtype %d is neither KAPPAGEN_F32 nor KAPPAGEN_F64", fn, dtype);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n < 0 || n > ((int64_t)1 << 40) || nbins < 2 || nbins > kHistMaxBins || !(dv > 0.0) || !std::isfinite(dv) ||
+        !domain_ok(kappa, 0.0) || (flags & ~(uint32_t)KAPPAGEN_U1_64)) {
+        set_error("%s: need 0 <= n <= 2^40, 2 <= nbins <= %d, dv > 0, kappa > 3/2, flags in {0, KAPPAGEN_U1_64}", fn, kHistMaxBins);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!hist) {
+        set_error("%s: NULL histogram", fn);
+        return KAPPAGEN_ENULL;
+    }
+    if (!aligned_to(hist, 8)) {
+        set_error("%s: histogram not 8-byte aligned", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    const PhiloxKeys K = philox_expand_keys(seed);
+    const bool u64 = (flags & KAPPAGEN_U1_64) != 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32) {
+        const Coef<float> C = host_coef_f32(kappa, 1.0, true);        // theta = 1 folded: the chain returns 2 |v|/theta
+        const float inv = (float)(0.5 / dv);
+        return u64 ? launch_hist<float, true>(n, offset, K, C, inv, nbins, hist, st)
+                   : launch_hist<float, false>(n, offset, K, C, inv, nbins, hist, st);
+    }
+    const Coef<double> C = host_coef_f64(kappa, 1.0);
+    return u64 ? launch_hist<double, true>(n, offset, K, C, 1.0 / dv, nbins, hist, st)
+               : launch_hist<double, false>(n, offset, K, C, 1.0 / dv, nbins, hist, st);
 }
 
 extern "C" int kappagen_words(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,

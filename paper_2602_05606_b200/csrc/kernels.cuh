@@ -332,6 +332,64 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
     }
 }
 
+// ---------------------------------------------------------------- kappagen_speed_histogram (paper test 2)
+// S1-S4 only: |v|/theta of each particle, binned with width dv; no velocity is written.  Counts go to
+// per-warp-slot replicas of the histogram in shared memory (most particles fall into the few bins around
+// |v| = theta, so one copy per block would serialise on a handful of addresses) and are flushed to the
+// caller's 64-bit counters once per block.  speed_over_theta: float: half of the packed chain's 2V with
+// theta = 1 folded in; double: speed_f64 with theta = 1.
+constexpr int kHistMaxBins = 4096;
+
+template <bool U64>
+__device__ __forceinline__ void group_speeds(uint64_t g0, const PhiloxKeys& K, const Coef<float>& C, float (&s)[4]) {
+    uint32_t w0[4], w1[4], w2[4], w3[4];
+    group_words<4>(g0, K, w0, w1, w2, w3);
+#pragma unroll
+    for (int e = 0; e < 4; e += 2) up2(speed2_f32x2<U64>(w0[e], w0[e + 1], w3[e], w3[e + 1], C), s[e], s[e + 1]);   // 2V
+}
+template <bool U64>
+__device__ __forceinline__ void group_speeds(uint64_t g0, const PhiloxKeys& K, const Coef<double>& C, double (&s)[2]) {
+    uint32_t w0[2], w1[2], w2[2], w3[2];
+    group_words<2>(g0, K, w0, w1, w2, w3);
+#pragma unroll
+    for (int e = 0; e < 2; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
+}
+__device__ __forceinline__ int bin_of(float s, float inv) { return __float2int_rz(s * inv); }     // saturating
+__device__ __forceinline__ int bin_of(double s, double inv) { return __double2int_rz(s * inv); }
+
+// inv = 1/dv (double) or 1/(2 dv) (float, whose chain returns 2V), rounded to T.
+template <typename T, bool U64>
+__global__ void __launch_bounds__(kThreads)
+speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
+                       T inv, int nbins, int replicas, unsigned long long* __restrict__ hist) {
+    extern __shared__ uint32_t sh_hist[];
+    constexpr int G = 16 / sizeof(T);
+    constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    for (int b = threadIdx.x; b < nbins * replicas; b += kThreads) sh_hist[b] = 0u;
+    __syncthreads();
+    uint32_t* mine = sh_hist + ((threadIdx.x >> 5) % (unsigned)replicas) * nbins;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+#pragma unroll
+        for (int j = 0; j < kGroups; ++j) {
+            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+            if (i < n) {
+                T s[G];
+                group_speeds<U64>(offset + (uint64_t)i, K, C, s);
+#pragma unroll
+                for (int e = 0; e < G; ++e) {
+                    if (i + e < n) atomicAdd(mine + min(bin_of(s[e], inv), nbins - 1), 1u);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += kThreads) {
+        unsigned long long c = 0ull;
+        for (int r = 0; r < replicas; ++r) c += sh_hist[r * nbins + b];
+        if (c != 0ull) atomicAdd(hist + b, c);
+    }
+}
+
 // ---------------------------------------------------------------- test hooks
 __global__ void __launch_bounds__(kThreads)
 words_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,

@@ -47,6 +47,8 @@ def lib() -> ctypes.CDLL:
         L.kappagen_sample_flags.argtypes = [i64, f64, f64, u64, u64, ci, ctypes.c_uint32, vp, vp, vp, vp]
         L.kappagen_words4.argtypes = [i64, u64, u64, vp, vp, vp, vp, vp]
         L.kappagen_velocity_of_words_u64.argtypes = [i64, vp, vp, vp, vp, f64, f64, ci, vp, vp, vp, vp]
+        L.kappagen_speed_histogram.argtypes = [i64, f64, u64, u64, ci, ctypes.c_uint32, f64, i32, vp, vp]
+        L.kappagen_relative_entropy.argtypes = [vp, i32, f64, f64, f64, ci, ctypes.POINTER(ctypes.c_double)]
         L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
         L.kappagen_sample_cells_moments.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, vp, sz, vp]
         L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
@@ -58,7 +60,7 @@ def lib() -> ctypes.CDLL:
         dp = ctypes.POINTER(ctypes.c_double)
         L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
         L.kappagen_last_error.restype = ctypes.c_char_p
-        for name in ("kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
+        for name in ("kappagen_speed_histogram", "kappagen_relative_entropy", "kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
                      "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version"):
             getattr(L, name).restype = ci
@@ -247,3 +249,23 @@ def velocity_of_words(w0, w1, w2, kappa: float, theta: float, dtype="f32", strea
     _check(lib().kappagen_velocity_of_words(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(), kappa, theta, code,
                                             vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
     return vx, vy, vz
+
+
+def speed_histogram(n: int, kappa: float, seed: int, offset: int = 0, dtype="f32", flags: int = 0, dv: float = 0.2,
+                    nbins: int = 512, hist=None, stream=None, device="cuda"):
+    """kappagen_speed_histogram: accumulates the counts of |v|/theta into `hist` (int64 device tensor holding
+    unsigned 64-bit counters, zeroed here when not given)."""
+    if hist is None:
+        hist = torch.zeros(nbins, dtype=torch.int64, device=device)
+    _check(lib().kappagen_speed_histogram(n, kappa, seed, offset, _dtype_code(dtype), flags, dv, nbins, hist.data_ptr(),
+                                          _stream(stream)))
+    return hist
+
+
+def relative_entropy(hist, kappa: float, dv: float = 0.2, eps: float = 1e-10, which: int = 0) -> float:
+    """kappagen_relative_entropy (Eq. 27) of a histogram (any integer tensor/array; copied to the host)."""
+    import numpy as np
+    h = np.ascontiguousarray(hist.cpu().numpy() if hasattr(hist, "cpu") else hist).astype(np.uint64)
+    out = ctypes.c_double(0.0)
+    _check(lib().kappagen_relative_entropy(h.ctypes.data, h.size, dv, kappa, eps, which, ctypes.byref(out)))
+    return out.value
