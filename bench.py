@@ -315,6 +315,12 @@ def extras(kg, torch, dtype):
                                                             stream=st, store=False), 5, 2, torch)
     k = sum(ms) / len(ms)
     out["cells_moments_only_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k}
+    # paper test 2 on the device: generate and bin 2^28 speeds, no velocity written
+    hist = torch.zeros(512, dtype=torch.int64, device="cuda")
+    for dt in ("f32", "f64"):
+        _, ms = time_launches(lambda s: kg.speed_histogram(n, 4.1, 1, s * n, dt, 0, 0.2, 512, hist=hist, stream=st), 5, 2, torch)
+        k = sum(ms) / len(ms)
+        out["speed_histogram_" + dt] = {"particles_per_s": n / (k * 1e-3), "ms": k}
     return out
 
 
