@@ -28,11 +28,11 @@ static inline size_t elem_size(int dtype) { return dtype == KAPPAGEN_F32 ? 4 : 8
 // Grid for a grid-stride kernel: enough blocks to fill every SM at the kernel's occupancy, never more
 // than there are tiles.  `blocks_per_sm` comes from the occupancy API, once per kernel and device.
 template <typename Kernel>
-static int grid_for(Kernel kernel, int64_t tiles, int* grid_out) {
+static int grid_for(Kernel kernel, int64_t tiles, int* grid_out, int threads = kThreads) {
     int dev = 0, sms = 0, per_sm = 0;
     KG_CUDA(cudaGetDevice(&dev));
     KG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    KG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0));
+    KG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0));
     if (per_sm < 1) per_sm = 1;
     const int64_t full = (int64_t)sms * per_sm;
     *grid_out = (int)(tiles < full ? tiles : full);
@@ -66,10 +66,11 @@ static int check_planes(const char* fn, int64_t n, int dtype, const void* vx, co
 template <typename T, bool VEC, bool FOLD, bool U64>
 static int launch_sample_as(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T* vx, T* vy, T* vz,
                             cudaStream_t st) {
-    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * TileTraits<T>::groups;
+    constexpr int threads = TileTraits<T>::threads;
+    constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
     int grid = 0, rc;
-    if ((rc = grid_for(sample_kernel<T, VEC, FOLD, U64>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
-    sample_kernel<T, VEC, FOLD, U64><<<grid, kThreads, 0, st>>>(n, offset, K, C, vx, vy, vz);
+    if ((rc = grid_for(sample_kernel<T, VEC, FOLD, U64>, (n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+    sample_kernel<T, VEC, FOLD, U64><<<grid, threads, 0, st>>>(n, offset, K, C, vx, vy, vz);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
 }

@@ -18,12 +18,14 @@ namespace kappagen {
 
 constexpr int kThreads = 256;
 constexpr int kGroups = 2;  // 128-bit groups per thread per tile
-// Tile shape of the sample kernels, measured on B200 (_F64 macros are sweep knobs).
-// double: 4 groups (8 particles) per thread generated in one straight line -- whole tiles only, stores
-// last -- under __launch_bounds__(256, 2): the chains are long, latency-bound and share 64-bit constants,
-// and 122 registers let the compiler keep those constants resident (1.05e11 particles/s against 9.1e10
-// for 2 separate groups at 80 registers).  float: 2 groups, each generated and stored on its own (joint
-// generation costs registers and 3 %); min-blocks 1 spelled out lets ptxas use 54 registers (+1 %).
+// Tile shape of the sample kernels, measured on B200 (the macros are sweep knobs).
+// double: 4 groups (8 particles) per thread generated in one straight line -- whole tiles inside one 2^32
+// block of counters only, one Philox head per tile, no branch between the groups, stores last -- with the
+// register budget of one 256-thread block per SM (162 registers): the chains are long and latency-bound
+// and share 64-bit constants, which the compiler keeps resident.  1.19e11 particles/s, against 9.1e10 for
+// 2 separately guarded groups at 80 registers; more warps per SM (128-thread blocks x 3, 384 x 1, 86
+// registers x 2) are all slower.  float: the same straight-line tile with 2 groups (8 particles, 96
+// registers): 2.29e11 particles/s; 1, 3 or 4 groups and min-blocks 2-4 are within 3 % below it.
 #ifndef KG_JOINT_F64
 #define KG_JOINT_F64 1
 #endif
@@ -31,12 +33,25 @@ constexpr int kGroups = 2;  // 128-bit groups per thread per tile
 #define KG_F64_GROUPS 4
 #endif
 #ifndef KG_F64_MINB
-#define KG_F64_MINB 2
+#define KG_F64_MINB 1
+#endif
+#ifndef KG_F64_THREADS
+#define KG_F64_THREADS 256
+#endif
+#ifndef KG_JOINT_F32
+#define KG_JOINT_F32 1
+#endif
+#ifndef KG_F32_GROUPS
+#define KG_F32_GROUPS 2
+#endif
+#ifndef KG_F32_MINB
+#define KG_F32_MINB 1
 #endif
 template <typename T> struct TileTraits {
-    static constexpr bool joint = (sizeof(T) == 8) && KG_JOINT_F64;
-    static constexpr int groups = sizeof(T) == 8 ? KG_F64_GROUPS : kGroups;   // of the sample kernel
-    static constexpr int minb = sizeof(T) == 8 ? KG_F64_MINB : 1;
+    static constexpr bool joint = (sizeof(T) == 8) ? KG_JOINT_F64 : KG_JOINT_F32;
+    static constexpr int groups = sizeof(T) == 8 ? KG_F64_GROUPS : KG_F32_GROUPS;   // of the sample kernel
+    static constexpr int minb = sizeof(T) == 8 ? KG_F64_MINB : KG_F32_MINB;
+    static constexpr int threads = sizeof(T) == 8 ? KG_F64_THREADS : kThreads;
 };
 
 template <typename T> struct Vec128;
@@ -69,13 +84,12 @@ __device__ __forceinline__ void group_words(uint64_t g0, const PhiloxKeys& K, ui
     }
 }
 
-// One 128-bit group: G consecutive particles starting at global counter g0.  float: two packed pairs
-// (math_f32x2.cuh, bit-identical to the scalar chain); double: two scalar chains.
-template <bool FOLD, bool U64 = false>
-__device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<float>& C,
-                                                 float (&ox)[4], float (&oy)[4], float (&oz)[4]) {
-    uint32_t w0[4], w1[4], w2[4], w3[4];
-    group_words<4>(g0, K, w0, w1, w2, w3);
+// Velocities of one 128-bit group from its words.  float: two packed pairs (math_f32x2.cuh, bit-identical
+// to the scalar chain); double: two scalar chains.
+template <bool FOLD, bool U64>
+__device__ __forceinline__ void words_to_velocities(const uint32_t (&w0)[4], const uint32_t (&w1)[4], const uint32_t (&w2)[4],
+                                                    const uint32_t (&w3)[4], const Coef<float>& C, float (&ox)[4],
+                                                    float (&oy)[4], float (&oz)[4]) {
 #pragma unroll
     for (int e = 0; e < 4; e += 2) {
         const uint32_t p0[2] = {w0[e], w0[e + 1]}, p1[2] = {w1[e], w1[e + 1]}, p2[2] = {w2[e], w2[e + 1]};
@@ -87,13 +101,30 @@ __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& 
         oz[e] = c[0]; oz[e + 1] = c[1];
     }
 }
-template <bool FOLD, bool U64 = false>
-__device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<double>& C,
-                                                 double (&ox)[2], double (&oy)[2], double (&oz)[2]) {
-    uint32_t w0[2], w1[2], w2[2], w3[2];
-    group_words<2>(g0, K, w0, w1, w2, w3);
+template <bool FOLD, bool U64>
+__device__ __forceinline__ void words_to_velocities(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
+                                                    const uint32_t (&w3)[2], const Coef<double>& C, double (&ox)[2],
+                                                    double (&oy)[2], double (&oz)[2]) {
 #pragma unroll
     for (int e = 0; e < 2; ++e) velocity_f64<U64>(w0[e], w1[e], w2[e], w3[e], C, ox[e], oy[e], oz[e]);
+}
+
+// One 128-bit group: G consecutive particles starting at global counter g0.
+template <bool FOLD, bool U64 = false, typename T, int G>
+__device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& K, const Coef<T>& C,
+                                                 T (&ox)[G], T (&oy)[G], T (&oz)[G]) {
+    uint32_t w0[G], w1[G], w2[G], w3[G];
+    group_words<G>(g0, K, w0, w1, w2, w3);
+    words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
+}
+// The same for a group known not to wrap its low counter word, given the shared head: no branch.
+template <bool FOLD, bool U64, typename T, int G>
+__device__ __forceinline__ void group_velocities_head(uint32_t lo, const PhiloxHead& H, const PhiloxKeys& K, const Coef<T>& C,
+                                                      T (&ox)[G], T (&oy)[G], T (&oz)[G]) {
+    uint32_t w0[G], w1[G], w2[G], w3[G];
+#pragma unroll
+    for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
+    words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
 }
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
@@ -129,7 +160,8 @@ template <typename T, bool VEC, bool FOLD, bool U64>
 __device__ __forceinline__ void tile_group(int64_t base, int j, int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C,
                                            T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     constexpr int G = 16 / sizeof(T);
-    const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+    constexpr int kT = TileTraits<T>::threads;
+    const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
     if (i < n) {
         T ox[G], oy[G], oz[G];
         group_velocities<FOLD, U64>(offset + (uint64_t)i, K, C, ox, oy, oz);
@@ -138,25 +170,29 @@ __device__ __forceinline__ void tile_group(int64_t base, int j, int64_t n, uint6
 }
 
 template <typename T, bool VEC, bool FOLD, bool U64>
-__global__ void __launch_bounds__(kThreads, TileTraits<T>::minb)
+__global__ void __launch_bounds__(TileTraits<T>::threads, TileTraits<T>::minb)
 sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
               T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
     constexpr int G = 16 / sizeof(T);
     constexpr int NG = TileTraits<T>::groups;
-    constexpr int64_t kTile = (int64_t)kThreads * G * NG;
+    constexpr int kT = TileTraits<T>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
-        if (VEC && TileTraits<T>::joint && base + kTile <= n) {
-            // whole tile in range: all groups of the thread in one straight line, so that their independent
-            // chains interleave and share the materialised constants; stores last
+        const uint64_t g_tile = offset + (uint64_t)base;
+        if (VEC && TileTraits<T>::joint && base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+            // whole tile in range and inside one 2^32 block of counters: one Philox head for the tile and all
+            // groups of the thread in one straight line -- no branch between them, so their independent chains
+            // interleave and share the materialised constants; stores last
+            const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             T ox[NG][G], oy[NG][G], oz[NG][G];
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
-                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
-                group_velocities<FOLD, U64>(offset + (uint64_t)i, K, C, ox[j], oy[j], oz[j]);
+                const uint32_t lo = (uint32_t)g_tile + (uint32_t)(j * (kT * G)) + threadIdx.x * (uint32_t)G;
+                group_velocities_head<FOLD, U64>(lo, H, K, C, ox[j], oy[j], oz[j]);
             }
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
-                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
                 store_group(vx + i, ox[j]);
                 store_group(vy + i, oy[j]);
                 store_group(vz + i, oz[j]);
