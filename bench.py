@@ -34,10 +34,10 @@ FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURE
 FALLBACK_SM_MHZ = 1965.0               # B200 maximum SM clock (MEASURED_PEAKS.json sm_max_mhz when present)
 N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one sample_kernel launch at 2^28 particles, and the busy
-# fraction of the limiting pipe, from the ncu --set full captures summarised in profiles/r01c_kernels.md.
-NCU_TRAFFIC_BYTES = {"f32": 3162542408, "f64": 6383231288}
-NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed", 79.2),
-                "f64": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 57.5)}
+# fraction of the limiting pipe, from the ncu --set full captures summarised in profiles/r01d_kernels.md.
+NCU_TRAFFIC_BYTES = {"f32": 3162292696, "f64": 6383364976}
+NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed", 77.4),
+                "f64": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 62.4)}
 # The sampler is bound by SM arithmetic, not by HBM.  Algorithmic work per particle on
 # the limiting pipe and that pipe's peak rate in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a
