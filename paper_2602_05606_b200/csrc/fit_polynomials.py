@@ -10,6 +10,7 @@ only: the CPU checker neither imports nor runs it, and nothing here is used at r
 """
 from __future__ import annotations
 
+import re
 import struct
 import sys
 
@@ -57,7 +58,8 @@ def r64(c):
 
 
 def hex32(c):
-    return float.hex(r32(c)) + "f"
+    m = re.match(r"(-?0x1\.)([0-9a-f]*?)0*(p[+-]\d+)$", float.hex(r32(c)))
+    return m.group(1) + (m.group(2) or "0") + m.group(3) + "f"
 
 
 def hex64(c):

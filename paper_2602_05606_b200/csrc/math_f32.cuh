@@ -18,7 +18,7 @@
 //   m = -log2(S)/kappa*            MUFU.LG2 when p = U1^(2/3) >= 1/4, else p G(p)/kappa* (degree-5 G)
 //   Y = 2^m - 1                    MUFU.EX2 when m >= 1/2, else m R(m) (degree-4 R)
 //   x = positive root of Eq. (24)  the printed form that adds, V = theta sqrt(x) = num rsqrt(num den)/2
-// The polynomial coefficients are near-minimax fits made by fit_polynomials.py (same directory).
+// The polynomial coefficients are the near-minimax fits printed by `fit_polynomials.py f32` (same directory).
 #pragma once
 #include <cstdint>
 #include "coefs.cuh"
@@ -56,22 +56,22 @@ __device__ __forceinline__ float speed2_f32(uint32_t w0, uint32_t w3, const Coef
     const float q1 = r + 1.0f;
     const float S = (t1 * q1) * mufu_rcp(q1 + p);                             // 1 - U1^(2/3), no cancellation
     // m = -log2(S)/kappa*.  For p < 1/4 (S -> 1) the MUFU result would carry only absolute accuracy:
-    // -log2(1-p) = p G(p), G of degree 5, relative error of the fit 3.7e-8 on [0, 1/4].
-    float G = 0x1.f5fc4cp-2f;
-    G = fmaf(G, p, 0x1.a938e2p-3f);
-    G = fmaf(G, p, 0x1.7cda04p-2f);
-    G = fmaf(G, p, 0x1.ebbc5ap-2f);
-    G = fmaf(G, p, 0x1.715672p-1f);
+    // -log2(1-p) = p G(p), G of degree 5, relative error of the fit 5.7e-8 on [0, 1/4].
+    float G = 0x1.f448fp-2f;
+    G = fmaf(G, p, 0x1.ab553ap-3f);
+    G = fmaf(G, p, 0x1.7c9f74p-2f);
+    G = fmaf(G, p, 0x1.ebc184p-2f);
+    G = fmaf(G, p, 0x1.71565ep-1f);
     G = fmaf(G, p, 0x1.715476p+0f);
     const float m_small = (p * C.s) * G;
     const float m_large = mufu_lg2(S) * -C.s;                                 // s = 1/kappa*
     const float m = (p < 0.25f) ? m_small : m_large;
-    // Y = 2^m - 1.  For m < 1/2 the subtraction would cancel: 2^m - 1 = m R(m), R of degree 4 (1.4e-8).
-    float R = 0x1.93f00ep-10f;
-    R = fmaf(R, m, 0x1.3823f8p-7f);
-    R = fmaf(R, m, 0x1.c6d326p-5f);
-    R = fmaf(R, m, 0x1.ebfb58p-3f);
-    R = fmaf(R, m, 0x1.62e430p-1f);
+    // Y = 2^m - 1.  For m < 1/2 the subtraction would cancel: 2^m - 1 = m R(m), R of degree 4 (2.7e-8).
+    float R = 0x1.945094p-10f;
+    R = fmaf(R, m, 0x1.3817fcp-7f);
+    R = fmaf(R, m, 0x1.c6d414p-5f);
+    R = fmaf(R, m, 0x1.ebfb52p-3f);
+    R = fmaf(R, m, 0x1.62e43p-1f);
     const float Y = (m < 0.5f) ? m * R : mufu_ex2(m) - 1.0f;
     // Eq. (24): root of b x^2 + A x - kappa* Y = 0, A = a + cL = a - c kappa* Y, in the form that adds
     const float A = fmaf(-C.ck, Y, C.a);
@@ -94,14 +94,14 @@ __device__ __forceinline__ void direction_f32(uint32_t w1, uint32_t w2, float& m
     // signed integer and re-centred, is simply (int32)(w2 << 2): q = ((int32)(w2 << 2) + 2) / 2^32.
     const float q = fmaf((float)(int32_t)(w2 << 2), 0x1p-32f, 0x1p-31f);
     const float z = q * q;
-    float sp = -0x1.2d9302p-8f;                                               // sin(pi q/2)/q, degree 3 in z (3.2e-9)
-    sp = fmaf(sp, z, 0x1.465e92p-4f);
+    float sp = -0x1.2d9b4p-8f;                                               // sin(pi q/2)/q, degree 3 in z (3.5e-8)
+    sp = fmaf(sp, z, 0x1.465ec4p-4f);
     sp = fmaf(sp, z, -0x1.4abbbap-1f);
     sp = fmaf(sp, z, 0x1.921fb6p+0f);
-    float cr = -0x1.4e35dap-6f;                                               // cos(pi q/2), degree 3 in z (3.3e-8)
-    cr = fmaf(cr, z, 0x1.03ae64p-2f);
-    cr = fmaf(cr, z, -0x1.3bd38cp+0f);
-    cr = fmaf(cr, z, 0x1.fffffep-1f);
+    float cr = -0x1.4e5e06p-6f;                                               // cos(pi q/2), degree 3 in z (6.0e-8)
+    cr = fmaf(cr, z, 0x1.03af58p-2f);
+    cr = fmaf(cr, z, -0x1.3bd392p+0f);
+    cr = fmaf(cr, z, 0x1.0p+0f);
     const float sr = sp * q;
     const uint32_t wq = w2 + 0x20000000u;                                     // k = wq >> 30 (k = 4 wraps to 0)
     const bool odd = (wq & 0x40000000u) != 0u;                                // k odd: swap

@@ -36,10 +36,10 @@ __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32
     const f32x2 p = mul2(r, r);
     const f32x2 q1 = add2(r, splat2(1.0f));
     const f32x2 S = mul2(mul2(t1, q1), KG_MAP2(mufu_rcp, add2(q1, p)));
-    f32x2 G = fma2(splat2(0x1.f5fc4cp-2f), p, splat2(0x1.a938e2p-3f));
-    G = fma2(G, p, splat2(0x1.7cda04p-2f));
-    G = fma2(G, p, splat2(0x1.ebbc5ap-2f));
-    G = fma2(G, p, splat2(0x1.715672p-1f));
+    f32x2 G = fma2(splat2(0x1.f448fp-2f), p, splat2(0x1.ab553ap-3f));
+    G = fma2(G, p, splat2(0x1.7c9f74p-2f));
+    G = fma2(G, p, splat2(0x1.ebc184p-2f));
+    G = fma2(G, p, splat2(0x1.71565ep-1f));
     G = fma2(G, p, splat2(0x1.715476p+0f));
     const f32x2 m_small = mul2(mul2(p, splat2(C.s)), G);
     const f32x2 m_large = mul2(KG_MAP2(mufu_lg2, S), splat2(-C.s));
@@ -47,10 +47,10 @@ __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32
     up2(p, pa, pb); up2(m_small, msa, msb); up2(m_large, mla, mlb);
     const float ma = (pa < 0.25f) ? msa : mla, mb = (pb < 0.25f) ? msb : mlb;
     const f32x2 m = pk2(ma, mb);
-    f32x2 R = fma2(splat2(0x1.93f00ep-10f), m, splat2(0x1.3823f8p-7f));
-    R = fma2(R, m, splat2(0x1.c6d326p-5f));
-    R = fma2(R, m, splat2(0x1.ebfb58p-3f));
-    R = fma2(R, m, splat2(0x1.62e430p-1f));
+    f32x2 R = fma2(splat2(0x1.945094p-10f), m, splat2(0x1.3817fcp-7f));
+    R = fma2(R, m, splat2(0x1.c6d414p-5f));
+    R = fma2(R, m, splat2(0x1.ebfb52p-3f));
+    R = fma2(R, m, splat2(0x1.62e43p-1f));
     const f32x2 y_small = mul2(m, R);
     const f32x2 y_large = add2(KG_MAP2(mufu_ex2, m), splat2(-1.0f));
     float ysa, ysb, yla, ylb;
@@ -93,12 +93,12 @@ __device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const
     const f32x2 sth = KG_MAP2(mufu_sqrt, fma2(ne, e, e));
     const f32x2 q = fma2(pk2((float)(int32_t)(w2[0] << 2), (float)(int32_t)(w2[1] << 2)), splat2(0x1p-32f), splat2(0x1p-31f));
     const f32x2 z = mul2(q, q);
-    f32x2 sp = fma2(splat2(-0x1.2d9302p-8f), z, splat2(0x1.465e92p-4f));
+    f32x2 sp = fma2(splat2(-0x1.2d9b4p-8f), z, splat2(0x1.465ec4p-4f));
     sp = fma2(sp, z, splat2(-0x1.4abbbap-1f));
     sp = fma2(sp, z, splat2(0x1.921fb6p+0f));
-    f32x2 cr = fma2(splat2(-0x1.4e35dap-6f), z, splat2(0x1.03ae64p-2f));
-    cr = fma2(cr, z, splat2(-0x1.3bd38cp+0f));
-    cr = fma2(cr, z, splat2(0x1.fffffep-1f));
+    f32x2 cr = fma2(splat2(-0x1.4e5e06p-6f), z, splat2(0x1.03af58p-2f));
+    cr = fma2(cr, z, splat2(-0x1.3bd392p+0f));
+    cr = fma2(cr, z, splat2(0x1.0p+0f));
     const f32x2 sr = mul2(sp, q);
     float sra, srb, cra, crb, ca, cb, sa, sb;
     up2(sr, sra, srb); up2(cr, cra, crb);
