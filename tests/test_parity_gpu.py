@@ -120,11 +120,12 @@ def test_theta_zero_and_status_codes():
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("offset", [2**32 - 1001, 2**32 - 2, 2**33 - 6, 2**64 - 5])
-def test_sample_parity_across_counter_carry(dtype, offset):
-    """The low counter word wraps inside a 128-bit group (odd offsets): the sampler's shared-head Philox
-    must fall back to the per-particle counter there (64-bit carry, reading R6)."""
-    n = 2003
+@pytest.mark.parametrize("offset,n", [(2**32 - 1001, 2003), (2**32 - 2, 2003), (2**33 - 6, 2003), (2**64 - 5, 2003),
+                                      (2**32 - 5001, 50_001), (2**32 - 4096, 40_960), (2**64 - 30_000, 60_000)])
+def test_sample_parity_across_counter_carry(dtype, offset, n):
+    """The low counter word wraps inside a 128-bit group (odd offsets) or inside a whole tile (the long cases):
+    the shared Philox head is only valid within one 2^32 block of counters, so the sampler must fall back to
+    the per-group and per-particle counters there (64-bit carry, reading R6)."""
     got = kg.sample(n, 2.5, 0.7, 9, offset, dtype)
     want = ref_sample(n, 2.5, 0.7, 9, offset % 2**64)
     err = max_rel_err(got, want)
