@@ -56,6 +56,8 @@ def parse_args():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / baseline / cells extra timings")
+    ap.add_argument("--sweep", action="store_true",
+                    help="also time kappagen_sample over 1e6 ... 2^30 particles and kappa 1.6 ... 10 (extras.sweep)")
     return ap.parse_args()
 
 
@@ -265,6 +267,8 @@ def run_ours(args):
         }
         if world == 1 and not args.no_extras:
             line["extras"] = extras(kg, torch, dtype)
+        if world == 1 and args.sweep:
+            line.setdefault("extras", {})["sweep"] = sweep(kg, torch)
         if world == 1:
             rate = oracle_rate(CPU_BASELINE_SAMPLE)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -321,6 +325,24 @@ def extras(kg, torch, dtype):
         _, ms = time_launches(lambda s: kg.speed_histogram(n, 4.1, 1, s * n, dt, 0, 0.2, 512, hist=hist, stream=st), 5, 2, torch)
         k = sum(ms) / len(ms)
         out["speed_histogram_" + dt] = {"particles_per_s": n / (k * 1e-3), "ms": k}
+    return out
+
+
+def sweep(kg, torch):
+    """The paper's benchmark shape (particles generated as a function of kappa) over the sizes the
+    north_star names: 1e6 ... 2^30 particles, kappa 1.6 ... 10, both dtypes (2^30 in fp32 only: 12.9 GB)."""
+    out = []
+    st = torch.cuda.current_stream()
+    for dt, tdt, sizes in (("f32", torch.float32, (10**6, 10**7, 10**8, 1 << 28, 1 << 30)),
+                           ("f64", torch.float64, (10**6, 10**7, 10**8, 1 << 28))):
+        planes = tuple(torch.empty(max(sizes), dtype=tdt, device="cuda") for _ in range(3))
+        for n in sizes:
+            view = tuple(p[:n] for p in planes)
+            for kappa in (1.6, 3.0, 10.0):
+                _, ms = time_launches(lambda s: kg.sample(n, kappa, 1.0, 1, s * n, dt, out=view, stream=st), 4, 2, torch)
+                k = min(ms)
+                out.append({"dtype": dt, "n": n, "kappa": kappa, "ms": k, "particles_per_s": n / (k * 1e-3)})
+        del planes
     return out
 
 
