@@ -79,6 +79,21 @@ def oracle_rate(n, offset=0):
     return n / (time.perf_counter() - t0)
 
 
+def oracle_rate_all_cores(n):
+    """The same oracle function over disjoint index ranges on every host core (counter-based, so the split is
+    trivial; ctypes releases the GIL).  Returns (particles/s, threads)."""
+    import concurrent.futures as cf
+    import oracle
+    cores = os.cpu_count() or 1
+    per = (n + cores - 1) // cores
+    oracle.lib()
+    t0 = time.perf_counter()
+    with cf.ThreadPoolExecutor(cores) as ex:
+        list(ex.map(lambda r: oracle.sample(min(per, n - r * per), KAPPA, THETA, SEED, r * per) if r * per < n else None,
+                    range(cores)))
+    return n / (time.perf_counter() - t0), cores
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -274,6 +289,9 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "first %d particles of configs[2] (kappa=2.0, theta=0.1, seed=42), "
                                               "oracle.sample in long double on one host thread" % CPU_BASELINE_SAMPLE}
+            rate_all, cores = oracle_rate_all_cores(4 * CPU_BASELINE_SAMPLE)
+            line["cpu_baseline"]["all_cores"] = {"value": rate_all, "unit": UNIT, "cores": cores,
+                                                 "sample": "first %d particles, split into %d index ranges" % (4 * CPU_BASELINE_SAMPLE, cores)}
         print(json.dumps(line))
     if world > 1:
         dist.barrier()

@@ -152,9 +152,16 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
                                                               (mode == kMomWarp || mode == kMomAtomic) ? mom : nullptr);
     KG_CUDA(cudaGetLastError());
     const int64_t n = ncell * (int64_t)ppc;
-    // floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1) for every i with i * ppc < 2^64 (i < n)
+    // cell_of(): a shift when ppc is a power of two; else floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1), exact for
+    // every i with i * ppc < 2^64 (i < n); else (~0) the plain 64-bit division
     const uint64_t up = (uint64_t)ppc;
-    const uint64_t magic = (up >= 2 && (uint64_t)n <= (~0ull) / up) ? (~0ull) / up + 1 : 0;
+    uint64_t magic = ~0ull;
+    if ((up & (up - 1)) == 0) {
+        magic = 0;
+        while ((1ull << magic) < up) ++magic;
+    } else if ((uint64_t)n <= (~0ull) / up) {
+        magic = (~0ull) / up + 1;                           // >= 2^32 > 64 for every ppc < 2^31
+    }
 #define KG_CELLS(V, S, M) launch_cells_as<T, V, S, M>(n, ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz, mom, mode, lanes, st)
     if (mom == nullptr) return vec ? KG_CELLS(true, true, false) : KG_CELLS(false, true, false);
     if (!store) return KG_CELLS(true, false, true);

@@ -239,10 +239,12 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
     W[cell] = C;
 }
 
-// floor(i / ppc) without a 64-bit division: magic = floor(2^64 / ppc) + 1 is exact for i * ppc < 2^64 (the
-// launcher checks n * ppc < 2^64 and passes magic = 0 otherwise, which selects the plain division).
+// floor(i / ppc) without a 64-bit division.  magic < 64: ppc = 2^magic, a shift.  Otherwise magic =
+// floor(2^64 / ppc) + 1, exact for i * ppc < 2^64 (the launcher checks n * ppc < 2^64 and passes magic = ~0
+// otherwise, which selects the plain division).
 __device__ __forceinline__ int64_t cell_of(int64_t i, uint32_t ppc, uint64_t magic) {
-    return magic ? (int64_t)__umul64hi((uint64_t)i, magic) : i / (int64_t)ppc;
+    if (magic < 64ull) return i >> (int)magic;
+    return magic != ~0ull ? (int64_t)__umul64hi((uint64_t)i, magic) : i / (int64_t)ppc;
 }
 
 template <typename T>
