@@ -52,6 +52,10 @@ template <typename T> struct TileTraits {
     static constexpr int groups = sizeof(T) == 8 ? KG_F64_GROUPS : KG_F32_GROUPS;   // of the sample kernel
     static constexpr int minb = sizeof(T) == 8 ? KG_F64_MINB : KG_F32_MINB;
     static constexpr int threads = sizeof(T) == 8 ? KG_F64_THREADS : kThreads;
+    // round 1's product M0 * lo32(g) of the thread's 2nd..8th particle by adding the constant M0 * distance to the
+    // first one's: two ALU adds instead of a quarter-rate multiply.  Pays where the FMA-heavy pipe is the
+    // bound (float: +1 %), costs where it is not (double: -5 %).
+    static constexpr bool round1_add = sizeof(T) == 4;
 };
 
 template <typename T> struct Vec128;
@@ -126,6 +130,16 @@ __device__ __forceinline__ void group_velocities_head(uint32_t lo, const PhiloxH
     for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
     words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
 }
+// q_first = M0 * lo32(counter of the thread's first particle in the tile); this group starts `delta` later.
+template <bool FOLD, bool U64, typename T, int G>
+__device__ __forceinline__ void group_velocities_head(uint64_t q_first, uint32_t delta, const PhiloxHead& H, const PhiloxKeys& K,
+                                                      const Coef<T>& C, T (&ox)[G], T (&oy)[G], T (&oz)[G]) {
+    uint32_t w0[G], w1[G], w2[G], w3[G];
+#pragma unroll
+    for (int e = 0; e < G; ++e)
+        particle_words_q0(q_first + (uint64_t)kPhiloxM0 * (uint64_t)(delta + (uint32_t)e), H, K, w0[e], w1[e], w2[e], w3[e]);
+    words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
+}
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
 __device__ __forceinline__ void store_group(float* p, const float (&v)[4]) {
@@ -184,11 +198,16 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
             // groups of the thread in one straight line -- no branch between them, so their independent chains
             // interleave and share the materialised constants; stores last
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)((uint32_t)g_tile + threadIdx.x * (uint32_t)G);
             T ox[NG][G], oy[NG][G], oz[NG][G];
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
-                const uint32_t lo = (uint32_t)g_tile + (uint32_t)(j * (kT * G)) + threadIdx.x * (uint32_t)G;
-                group_velocities_head<FOLD, U64>(lo, H, K, C, ox[j], oy[j], oz[j]);
+                if constexpr (TileTraits<T>::round1_add) {
+                    group_velocities_head<FOLD, U64>(q_first, (uint32_t)(j * (kT * G)), H, K, C, ox[j], oy[j], oz[j]);
+                } else {
+                    const uint32_t lo = (uint32_t)g_tile + (uint32_t)(j * (kT * G)) + threadIdx.x * (uint32_t)G;
+                    group_velocities_head<FOLD, U64>(lo, H, K, C, ox[j], oy[j], oz[j]);
+                }
             }
 #pragma unroll
             for (int j = 0; j < NG; ++j) {

@@ -68,10 +68,17 @@ __device__ __forceinline__ PhiloxHead philox_head(uint32_t g_hi, const PhiloxKey
     return PhiloxHead{(uint32_t)(p >> 32), (uint32_t)p};
 }
 // Same words as particle_words(g, ...) for g = (g_hi << 32) | g_lo, given H = philox_head(g_hi, K).
+// q0 = M0 * lo32(g), round 1's only product, supplied by the caller: for counters a compile-time distance
+// apart it is one multiply plus 64-bit additions of constants (M0 (g + d) = M0 g + M0 d).
+__device__ __forceinline__ void particle_words_q0(uint64_t q0, const PhiloxHead& H, const PhiloxKeys& K,
+                                                  uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3);
 __device__ __forceinline__ void particle_words_head(uint32_t g_lo, const PhiloxHead& H, const PhiloxKeys& K,
                                                     uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3) {
+    particle_words_q0((uint64_t)kPhiloxM0 * (uint64_t)g_lo, H, K, w0, w1, w2, w3);
+}
+__device__ __forceinline__ void particle_words_q0(uint64_t q0, const PhiloxHead& H, const PhiloxKeys& K,
+                                                  uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3) {
     // round 1 (c2 = c3 = 0): c = (g_hi ^ k0[0], 0, hi(M0 g_lo) ^ k1[0], lo(M0 g_lo))
-    const uint64_t q0 = (uint64_t)kPhiloxM0 * (uint64_t)g_lo;
     // round 2: the M0 product is the shared head; c1 = 0
     const uint64_t q1 = (uint64_t)kPhiloxM1 * (uint64_t)((uint32_t)(q0 >> 32) ^ K.k1[0]);
     uint32_t c0 = (uint32_t)(q1 >> 32) ^ K.k0[1];
