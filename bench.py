@@ -54,7 +54,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--dtype", choices=["f32", "f64"], default="f32")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / baseline / cells extra timings")
     ap.add_argument("--sweep", action="store_true",
                     help="also time kappagen_sample over 1e6 ... 2^30 particles and kappa 1.6 ... 10 (extras.sweep)")
@@ -235,8 +235,11 @@ def run_ours(args):
     kg.sample_host(n, KAPPA, THETA, SEED, rank * n, dtype, out=host)            # warm-up (also faults the pages in)
     barrier()
     t0 = time.perf_counter()
+    e2e_each = []
     for s in range(args.e2e_steps):
-        kg.sample_host(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, out=host)
+        t1 = time.perf_counter()
+        kg.sample_host(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, out=host)   # synchronous
+        e2e_each.append(time.perf_counter() - t1)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -270,7 +273,8 @@ def run_ours(args):
             "dtype": dtype, "data": "synthetic", "config": config_dict(dtype, world),
             "clocks": clocks, "gpu_launches": args.steps,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 3 * es * n * world,
-                    "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum},
+                    "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum,
+                    "ms_per_step": [round(1e3 * t, 3) for t in e2e_each]},
             "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": alu_unit,
                          "frac": alu_achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES[dtype], "pipe": pipe,
                          "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5)" % (N_SM, per_clk, sm_mhz),
