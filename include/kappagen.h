@@ -18,7 +18,9 @@
  *    and allocates nothing that outlives a call.
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device-buffer
  *    calls enqueue on `stream` and return without synchronising; argument errors are returned
- *    at once, asynchronous CUDA errors surface at the caller's next synchronisation.
+ *    at once, asynchronous CUDA errors surface at the caller's next synchronisation.  They
+ *    allocate nothing and only launch kernels, so they may be recorded by stream capture into a
+ *    CUDA graph (kappagen_sample_host may not: it allocates staging buffers and synchronises).
  *  - Output planes are SoA: vx[i], vy[i], vz[i]; element type float (KAPPAGEN_F32) or double
  *    (KAPPAGEN_F64).  Planes must be aligned to the element size; 16-byte aligned planes take
  *    the vector-store path, others a scalar-store path that writes the same values.
