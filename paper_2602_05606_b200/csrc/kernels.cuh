@@ -25,7 +25,7 @@ constexpr int kGroups = 2;  // 128-bit groups per thread per tile
 // and share 64-bit constants, which the compiler keeps resident.  1.19e11 particles/s, against 9.1e10 for
 // 2 separately guarded groups at 80 registers; more warps per SM (128-thread blocks x 3, 384 x 1, 86
 // registers x 2) are all slower.  float: the same straight-line tile with 2 groups (8 particles, 96
-// registers): 2.29e11 particles/s; 1, 3 or 4 groups and min-blocks 2-4 are within 3 % below it.
+// registers): 2.31e11 particles/s; 1, 3 or 4 groups and min-blocks 2-4 are within 3 % below it.
 #ifndef KG_JOINT_F64
 #define KG_JOINT_F64 1
 #endif
@@ -335,7 +335,57 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                     int mom_lanes) {
     constexpr int G = 16 / sizeof(T);
     constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    const bool whole_groups = ppc % (uint32_t)G == 0u;                 // every 128-bit group inside one cell
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        const uint64_t g_tile = offset + (uint64_t)base;
+        if (VEC && whole_groups && base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+            // whole tile in range and inside one 2^32 block of counters: the straight-line tile of the
+            // uniform sampler (one Philox head; float: round-1 products by constant additions), one Coef per group
+            const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)((uint32_t)g_tile + threadIdx.x * (uint32_t)G);
+            T ox[kGroups][G], oy[kGroups][G], oz[kGroups][G];
+#pragma unroll
+            for (int j = 0; j < kGroups; ++j) {
+                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                const int64_t cell0 = cell_of(i, ppc, magic);
+                const Coef<T> C = W[cell0];
+                if constexpr (TileTraits<T>::round1_add)
+                    group_velocities_head<false, false>(q_first, (uint32_t)(j * (kThreads * G)), H, K, C, ox[j], oy[j], oz[j]);
+                else
+                    group_velocities_head<false, false>((uint32_t)(offset + (uint64_t)i), H, K, C, ox[j], oy[j], oz[j]);
+                if (drift != nullptr) {
+                    const T* d = drift + 3 * cell0 * drift_stride;
+                    const T dx = d[0], dy = d[1], dz = d[2];
+#pragma unroll
+                    for (int e = 0; e < G; ++e) {
+                        ox[j][e] += dx;
+                        oy[j][e] += dy;
+                        oz[j][e] += dz;
+                    }
+                }
+                if (MOM) {
+                    T ps[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll
+                    for (int e = 0; e < G; ++e) {
+                        ps[0] += ox[j][e];
+                        ps[1] += oy[j][e];
+                        ps[2] += oz[j][e];
+                        ps[3] = fma(ox[j][e], ox[j][e], fma(oy[j][e], oy[j][e], fma(oz[j][e], oz[j][e], ps[3])));
+                    }
+                    moments_out(ps, cell0, mom_mode, mom_lanes, mom);
+                }
+            }
+            if (STORE) {
+#pragma unroll
+                for (int j = 0; j < kGroups; ++j) {
+                    const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                    store_group(vx + i, ox[j]);
+                    store_group(vy + i, oy[j]);
+                    store_group(vz + i, oz[j]);
+                }
+            }
+            continue;
+        }
 #pragma unroll
         for (int j = 0; j < kGroups; ++j) {
             const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
