@@ -461,6 +461,24 @@ __device__ __forceinline__ void group_speeds(uint64_t g0, const PhiloxKeys& K, c
 #pragma unroll
     for (int e = 0; e < 2; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
 }
+// Speeds of one group from precomputed round-1 products (whole-tile path, see sample_kernel).
+template <bool U64, bool ADD, typename T, int G>
+__device__ __forceinline__ void group_speeds_head(uint64_t q_first, uint32_t lo_first, uint32_t delta, const PhiloxHead& H,
+                                                  const PhiloxKeys& K, const Coef<T>& C, T (&s)[G]) {
+    uint32_t w0[G], w1[G], w2[G], w3[G];
+#pragma unroll
+    for (int e = 0; e < G; ++e) {
+        if (ADD) particle_words_q0(q_first + (uint64_t)kPhiloxM0 * (uint64_t)(delta + (uint32_t)e), H, K, w0[e], w1[e], w2[e], w3[e]);
+        else particle_words_head(lo_first + delta + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
+    }
+    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int e = 0; e < G; e += 2) up2(speed2_f32x2<U64>(w0[e], w0[e + 1], w3[e], w3[e + 1], C), s[e], s[e + 1]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < G; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
+    }
+}
 __device__ __forceinline__ int bin_of(float s, float inv) { return __float2int_rz(s * inv); }     // saturating
 __device__ __forceinline__ int bin_of(double s, double inv) { return __double2int_rz(s * inv); }
 
@@ -476,6 +494,23 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
     __syncthreads();
     uint32_t* mine = sh_hist + ((threadIdx.x >> 5) % (unsigned)replicas) * nbins;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        const uint64_t g_tile = offset + (uint64_t)base;
+        if (base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+            // whole tile in range and inside one 2^32 block of counters: straight line, one Philox head
+            const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
+            const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
+            T s[kGroups][G];
+#pragma unroll
+            for (int j = 0; j < kGroups; ++j)
+                group_speeds_head<U64, TileTraits<T>::round1_add>(q_first, lo_first, (uint32_t)(j * (kThreads * G)), H, K, C, s[j]);
+#pragma unroll
+            for (int j = 0; j < kGroups; ++j) {
+#pragma unroll
+                for (int e = 0; e < G; ++e) atomicAdd(mine + min(bin_of(s[j][e], inv), nbins - 1), 1u);
+            }
+            continue;
+        }
 #pragma unroll
         for (int j = 0; j < kGroups; ++j) {
             const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
