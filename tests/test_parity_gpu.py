@@ -182,3 +182,21 @@ def test_config3_full_size_sampled_parity(cfg):
     sp2 = got[0].double() ** 2 + got[1].double() ** 2 + got[2].double() ** 2
     xmax = oracle.x_of_w0([2**32 - 1], cfg.kappa)[0] * cfg.theta**2
     assert torch.isfinite(sp2).all() and sp2.max().item() <= xmax * (1 + 1e-5) and sp2.min().item() > 0
+
+
+# ------------------------------------------------------------------ the whole accepted kappa range (reading R14)
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("kappa", [1.5001, 1.51, 25.0, 1e3, 1e6])
+def test_edge_words_at_the_ends_of_the_kappa_range(kappa, dtype):
+    """kappa just above 3/2 (kappa* -> 1: the heaviest admissible tail) and far beyond the fitted range
+    (kappa -> infinity: the Maxwellian limit, a -> 0.827): still within tolerance over the
+    whole 32-bit range of every word, and finite."""
+    w0 = wl.edge_words()
+    w1, w2 = w0[::-1].copy(), np.roll(w0, 7)
+    t = [torch.from_numpy(w.view(np.int32)).cuda() for w in (w0, w1, w2)]
+    got = kg.velocity_of_words(t[0], t[1], t[2], kappa, 0.7, dtype)
+    want = oracle.velocity_of_words(w0, w1, w2, kappa, 0.7)
+    err = max_rel_err(got, want)
+    report(test="kappa_range", kappa=kappa, dtype=dtype, max_rel_err=err)
+    assert err <= TOL[dtype], err
+    assert all(bool(torch.isfinite(g).all()) for g in got)
