@@ -274,7 +274,8 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": args.steps,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 3 * es * n * world,
                     "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum,
-                    "ms_per_step": [round(1e3 * t, 3) for t in e2e_each]},
+                    "ms_per_step": [round(1e3 * t, 3) for t in e2e_each],
+                    "value_at_median_step": world * n / sorted(e2e_each)[len(e2e_each) // 2]},
             "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": alu_unit,
                          "frac": alu_achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES[dtype], "pipe": pipe,
                          "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5)" % (N_SM, per_clk, sm_mhz),
