@@ -198,6 +198,11 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2602_05606_b200 import build as kbuild
+    if rank == 0:
+        kbuild.build()                                  # no-op when the in-tree library is up to date
+    if world > 1:
+        dist.barrier()
     kg.lib()                                            # fail loudly now if libkappagen.so is missing
     dtype, n = args.dtype, N_STEP
     tdt = torch.float32 if dtype == "f32" else torch.float64

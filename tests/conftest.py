@@ -26,3 +26,10 @@ def read_facts():
 @pytest.fixture(scope="session")
 def facts():
     return read_facts()
+
+
+@pytest.fixture(scope="session", autouse=True)
+def built_library():
+    """libkappagen.so is built in-tree (nvcc cross-compiles without a GPU); a no-op when it is up to date."""
+    from paper_2602_05606_b200 import build as kbuild
+    return kbuild.build()
