@@ -107,3 +107,27 @@ def test_relative_entropy_falls_like_one_over_n_then_meets_the_plateau():
     assert D[2**28] == pytest.approx(plateau, rel=0.5)
     # against its OWN distribution G the generator keeps converging (it samples G, not F: PAPER.md:201)
     assert kg.relative_entropy(acc, kappa, DV, 1e-10, 1) < 0.05 * plateau
+
+
+def test_kappa3_plateau_appears_beyond_1e10_particles():
+    """'The Monte Carlo results with kappa = 3.0 are indistinguishable from the Kappa distribution in Fig. 6.
+    Extrapolating the results toward the asymptotic value, we will see a difference when N_p >~ 10^9.5'
+    (PAPER.md:215).  The device histogram makes that regime cheap: 2^36 = 6.9e10 particles in a quarter of a
+    second.  D keeps falling through 2^30 (still noise) and settles on the plateau sum P_F ln(P_F/P_G) = 5.3e-8."""
+    kappa, nbins = 3.0, 128                      # |v| < 25.4 theta + open bin: every bin well populated at 2^30
+    acc = torch.zeros(nbins, dtype=torch.int64, device="cuda")
+    D, done = {}, 0
+    for total in (2**26, 2**30, 2**34, 2**36):
+        while done < total:
+            m = min(2**28, total - done)
+            kg.speed_histogram(m, kappa, 2, done, "f32", 0, DV, nbins, hist=acc)
+            done += m
+        assert int(acc.sum()) == total
+        D[total] = kg.relative_entropy(acc, kappa, DV, 1e-10, 0)
+    PF = oracle.bin_probabilities(kappa, DV, nbins, "exact")
+    PG = oracle.bin_probabilities(kappa, DV, nbins, "approx")
+    plateau = float(np.sum(PF * np.log(PF / PG)))
+    report(test="fig6_kappa3", D={str(k): v for k, v in D.items()}, plateau=plateau)
+    assert D[2**26] > 5 * plateau                         # particle noise hides the approximation
+    assert D[2**36] == pytest.approx(plateau, rel=0.25)   # ... until N_p ~ 1e10.5
+    assert D[2**34] < 2.5 * plateau
