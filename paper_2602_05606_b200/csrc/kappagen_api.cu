@@ -322,7 +322,8 @@ static int words_impl(const char* fn, int64_t n, uint64_t seed, uint64_t offset,
 template <typename T, bool U64>
 static int launch_hist(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T inv, int nbins,
                        unsigned long long* hist, cudaStream_t st) {
-    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    static_assert(TileTraits<T>::threads == kThreads, "the histogram kernel uses kThreads per block");
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * TileTraits<T>::groups;
     int replicas = (48 * 1024) / (nbins * 4);
     if (replicas > kThreads / 32) replicas = kThreads / 32;
     if (replicas < 1) replicas = 1;

@@ -484,12 +484,13 @@ __device__ __forceinline__ int bin_of(double s, double inv) { return __double2in
 
 // inv = 1/dv (double) or 1/(2 dv) (float, whose chain returns 2V), rounded to T.
 template <typename T, bool U64>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, TileTraits<T>::minb)
 speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
                        T inv, int nbins, int replicas, unsigned long long* __restrict__ hist) {
     extern __shared__ uint32_t sh_hist[];
     constexpr int G = 16 / sizeof(T);
-    constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
+    constexpr int NG = TileTraits<T>::groups;            // the sample kernel's tile shape: same chains, same trade-off
+    constexpr int64_t kTile = (int64_t)kThreads * G * NG;
     for (int b = threadIdx.x; b < nbins * replicas; b += kThreads) sh_hist[b] = 0u;
     __syncthreads();
     uint32_t* mine = sh_hist + ((threadIdx.x >> 5) % (unsigned)replicas) * nbins;
@@ -500,19 +501,19 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
             const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
-            T s[kGroups][G];
+            T s[NG][G];
 #pragma unroll
-            for (int j = 0; j < kGroups; ++j)
+            for (int j = 0; j < NG; ++j)
                 group_speeds_head<U64, TileTraits<T>::round1_add>(q_first, lo_first, (uint32_t)(j * (kThreads * G)), H, K, C, s[j]);
 #pragma unroll
-            for (int j = 0; j < kGroups; ++j) {
+            for (int j = 0; j < NG; ++j) {
 #pragma unroll
                 for (int e = 0; e < G; ++e) atomicAdd(mine + min(bin_of(s[j][e], inv), nbins - 1), 1u);
             }
             continue;
         }
 #pragma unroll
-        for (int j = 0; j < kGroups; ++j) {
+        for (int j = 0; j < NG; ++j) {
             const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
             if (i < n) {
                 T s[G];
