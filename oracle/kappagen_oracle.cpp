@@ -29,7 +29,10 @@
 //     cancel, the azimuth reduced to |angle| <= pi/4 on the integer word).  This is the
 //     function GPU parity is measured against.
 // tests/test_oracle_*.py pin both to the paper (Philox KATs, printed parameter facts, round
-// trip through Eq. (A11), exact CDF Eq. (3), Eq. (5), 50-digit mpmath evaluation of Table I).
+// trip through Eq. (A11), exact CDF Eq. (3), Eq. (5), 50-digit mpmath evaluation of Table I);
+// the literal evaluator (x_literal, dir_literal, oracle_sample_literal) in tests/test_oracle_literal.py
+// (Table I lines 5-10 typed once more in 50-digit mpmath; agreement with oracle_sample in the bulk;
+// polar axis and the (cos, sin) assignment from the top bits of the words).
 //
 // Parity status: every exported function below is pinned; none is "parity unpinned".
 
