@@ -140,6 +140,21 @@ int kappagen_velocity_of_words_u64(int64_t n, const uint32_t* w0, const uint32_t
                                    const uint32_t* w3, double kappa, double theta, int dtype,
                                    void* vx, void* vy, void* vz, void* stream);
 
+/* Test hooks through the code the samplers SHIP.  kappagen_sample runs whole tiles (256 threads x 8 particles per
+ * thread inside one 2^32 block of counters) through a path of its own: one shared Philox head per tile, round 1's
+ * product by constant additions (float), packed pairs of particles (float) / eight interleaved chains (double).
+ *  kappagen_words_tile: the four words of particles offset .. offset+n-1 drawn by the same tile walk, the same
+ *    whole-tile test and the same device functions as kappagen_sample's kernel for `dtype` (the two dtypes use
+ *    different tile shapes); w0..w3: device, [n] uint32 each, all required.
+ *  kappagen_velocity_of_words_tile: S2-S6 on caller-chosen words through that kernel's straight-line tile body
+ *    (same instantiation, words read from memory instead of drawn); flags = 0 or KAPPAGEN_U1_64 (then w3 is
+ *    required, otherwise ignored and may be NULL).  Any n; planes need only element alignment. */
+int kappagen_words_tile(int64_t n, uint64_t seed, uint64_t offset, int dtype,
+                        uint32_t* w0, uint32_t* w1, uint32_t* w2, uint32_t* w3, void* stream);
+int kappagen_velocity_of_words_tile(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                    const uint32_t* w3, double kappa, double theta, int dtype, uint32_t flags,
+                                    void* vx, void* vy, void* vz, void* stream);
+
 /* Paper test 2 on the device: generate n particles and count
  * their speeds |v|/theta in bins of width dv ("Delta v = 1/5") WITHOUT writing a velocity: S1-S4 only, in
  * the arithmetic of `dtype`, so 2^34 particles and more are a matter of milliseconds per 2^28.

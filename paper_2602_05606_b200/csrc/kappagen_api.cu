@@ -26,15 +26,25 @@ static inline bool aligned_to(const void* p, size_t a) { return (reinterpret_cas
 static inline size_t elem_size(int dtype) { return dtype == KAPPAGEN_F32 ? 4 : 8; }
 
 // Grid for a grid-stride kernel: enough blocks to fill every SM at the kernel's occupancy, never more
-// than there are tiles.  `blocks_per_sm` comes from the occupancy API, once per kernel and device.
-template <typename Kernel>
-static int grid_for(Kernel kernel, int64_t tiles, int* grid_out, int threads = kThreads) {
-    int dev = 0, sms = 0, per_sm = 0;
+// than there are tiles.  The (SM count, blocks per SM) pair is queried once per kernel instantiation, device and
+// launch shape (a function-local cache: the kernel is a template argument, so there is one cache per kernel instantiation), not on every launch --
+// small calls are launch-bound.
+template <auto Kernel>
+static int grid_for(int64_t tiles, int* grid_out, int threads = kThreads, size_t dyn_smem = 0) {
+    constexpr int kMaxDev = 64;
+    struct Entry { int sms, per_sm, threads; size_t smem; };
+    static thread_local Entry cache[kMaxDev] = {};
+    int dev = 0;
     KG_CUDA(cudaGetDevice(&dev));
-    KG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    KG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0));
-    if (per_sm < 1) per_sm = 1;
-    const int64_t full = (int64_t)sms * per_sm;
+    Entry local = {};
+    Entry& e = (dev >= 0 && dev < kMaxDev) ? cache[dev] : local;
+    if (e.sms == 0 || e.threads != threads || e.smem != dyn_smem) {
+        int sms = 0, per_sm = 0;
+        KG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        KG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, Kernel, threads, dyn_smem));
+        e = Entry{sms, per_sm < 1 ? 1 : per_sm, threads, dyn_smem};
+    }
+    const int64_t full = (int64_t)e.sms * e.per_sm;
     *grid_out = (int)(tiles < full ? tiles : full);
     return KAPPAGEN_OK;
 }
@@ -69,7 +79,7 @@ static int launch_sample_as(int64_t n, uint64_t offset, const PhiloxKeys& K, con
     constexpr int threads = TileTraits<T>::threads;
     constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
     int grid = 0, rc;
-    if ((rc = grid_for(sample_kernel<T, VEC, FOLD, U64>, (n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+    if ((rc = grid_for<sample_kernel<T, VEC, FOLD, U64>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
     sample_kernel<T, VEC, FOLD, U64><<<grid, threads, 0, st>>>(n, offset, K, C, vx, vy, vz);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
@@ -127,7 +137,7 @@ static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint64_t offs
                            cudaStream_t st) {
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
     int grid = 0, rc;
-    if ((rc = grid_for(sample_cells_kernel<T, VEC, STORE, MOM>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
+    if ((rc = grid_for<sample_cells_kernel<T, VEC, STORE, MOM>>((n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
     sample_cells_kernel<T, VEC, STORE, MOM><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride,
                                                                       vx, vy, vz, mom, mode, lanes);
     KG_CUDA(cudaGetLastError());
@@ -178,7 +188,7 @@ static int launch_mt(int64_t n, double kappa, double theta, uint64_t offset, con
     P.cp = (T)(1.0 / sqrt(9.0 * d));
     P.scale = (T)(theta * sqrt(0.5 * kappa));
     int grid = 0, rc;
-    if ((rc = grid_for(baseline_mt_kernel<T>, (n + kThreads - 1) / kThreads, &grid)) != KAPPAGEN_OK) return rc;
+    if ((rc = grid_for<baseline_mt_kernel<T>>((n + kThreads - 1) / kThreads, &grid)) != KAPPAGEN_OK) return rc;
     baseline_mt_kernel<T><<<grid, kThreads, 0, st>>>(n, offset, K, P, vx, vy, vz, trips);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
@@ -313,7 +323,7 @@ static int words_impl(const char* fn, int64_t n, uint64_t seed, uint64_t offset,
         return KAPPAGEN_EALIGN;
     }
     int grid = 0, rc;
-    if ((rc = grid_for(words_kernel, (n + 4 * kThreads - 1) / (4 * kThreads), &grid)) != KAPPAGEN_OK) return rc;
+    if ((rc = grid_for<words_kernel>((n + 4 * kThreads - 1) / (4 * kThreads), &grid)) != KAPPAGEN_OK) return rc;
     words_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(n, offset, philox_expand_keys(seed), w0, w1, w2, w3);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
@@ -327,10 +337,25 @@ static int launch_hist(int64_t n, uint64_t offset, const PhiloxKeys& K, const Co
     int replicas = (48 * 1024) / (nbins * 4);
     if (replicas > kThreads / 32) replicas = kThreads / 32;
     if (replicas < 1) replicas = 1;
+    const size_t smem = (size_t)replicas * nbins * 4;
     int grid = 0, rc;
-    if ((rc = grid_for(speed_histogram_kernel<T, U64>, (n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
-    speed_histogram_kernel<T, U64><<<grid, kThreads, (size_t)replicas * nbins * 4, st>>>(n, offset, K, C, inv, nbins, replicas, hist);
-    KG_CUDA(cudaGetLastError());
+    // The block counts into 32-bit shared-memory replicas and flushes them once at its end.  A replica sees the
+    // particles of ceil(warps/replicas) of the block's 8 warps, so per launch a block may process at most
+    // 2^32 / that share of its particles: split larger calls into launches of `cap` particles (whatever the
+    // device's SM count or the occupancy), each flushing into the caller's 64-bit counters.
+    const int64_t tiles_all = (n + tile - 1) / tile;
+    if ((rc = grid_for<speed_histogram_kernel<T, U64>>(tiles_all, &grid, kThreads, smem)) != KAPPAGEN_OK) return rc;
+    const int warps = kThreads / 32, share = (warps + replicas - 1) / replicas;
+    const int64_t per_block = (((int64_t)1 << 32) - 1) / share * warps / tile * tile;     // particles, whole tiles
+    const int64_t cap = per_block * (int64_t)(grid < 1 ? 1 : grid) / 2;                   // factor 2: uneven tile counts per block
+    for (int64_t done = 0; done < n;) {
+        const int64_t m = (n - done) < cap ? (n - done) : cap;
+        int g = 0;
+        if ((rc = grid_for<speed_histogram_kernel<T, U64>>((m + tile - 1) / tile, &g, kThreads, smem)) != KAPPAGEN_OK) return rc;
+        speed_histogram_kernel<T, U64><<<g, kThreads, smem, st>>>(m, offset + (uint64_t)done, K, C, inv, nbins, replicas, hist);
+        KG_CUDA(cudaGetLastError());
+        done += m;
+    }
     return KAPPAGEN_OK;
 }
 
@@ -402,14 +427,14 @@ static int velocity_of_words_impl(const char* fn, int64_t n, const uint32_t* w0,
         const bool fold = theta_folds(theta);              // the same choice kappagen_sample makes
         const Coef<float> C = host_coef_f32(kappa, theta, fold);
         if (fold) {
-            if ((rc = grid_for(velocity_of_words_kernel<float, true, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            if ((rc = grid_for<velocity_of_words_kernel<float, true, U64>>(tiles, &grid)) != KAPPAGEN_OK) return rc;
             velocity_of_words_kernel<float, true, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, C, (float*)vx, (float*)vy, (float*)vz);
         } else {
-            if ((rc = grid_for(velocity_of_words_kernel<float, false, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+            if ((rc = grid_for<velocity_of_words_kernel<float, false, U64>>(tiles, &grid)) != KAPPAGEN_OK) return rc;
             velocity_of_words_kernel<float, false, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, C, (float*)vx, (float*)vy, (float*)vz);
         }
     } else {
-        if ((rc = grid_for(velocity_of_words_kernel<double, false, U64>, tiles, &grid)) != KAPPAGEN_OK) return rc;
+        if ((rc = grid_for<velocity_of_words_kernel<double, false, U64>>(tiles, &grid)) != KAPPAGEN_OK) return rc;
         velocity_of_words_kernel<double, false, U64><<<grid, kThreads, 0, st>>>(n, w0, w1, w2, w3, host_coef_f64(kappa, theta),
                                                                                 (double*)vx, (double*)vy, (double*)vz);
     }
@@ -429,6 +454,84 @@ extern "C" int kappagen_velocity_of_words_u64(int64_t n, const uint32_t* w0, con
                                               void* vz, void* stream) {
     return velocity_of_words_impl<true>("kappagen_velocity_of_words_u64", n, w0, w1, w2, w3, kappa, theta, dtype, vx, vy, vz,
                                         stream);
+}
+
+// ---- test hooks that go through the code the samplers ship (whole-tile path), include/kappagen.h
+template <typename T>
+static int launch_words_tile(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2, uint32_t* w3,
+                             cudaStream_t st) {
+    constexpr int threads = TileTraits<T>::threads;
+    constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
+    int grid = 0, rc;
+    if ((rc = grid_for<words_tile_kernel<T>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+    words_tile_kernel<T><<<grid, threads, 0, st>>>(n, offset, philox_expand_keys(seed), w0, w1, w2, w3);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_words_tile(int64_t n, uint64_t seed, uint64_t offset, int dtype, uint32_t* w0, uint32_t* w1,
+                                   uint32_t* w2, uint32_t* w3, void* stream) {
+    const char* fn = "kappagen_words_tile";
+    if (n < 0 || (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64)) {
+        set_error("%s: negative count or bad dtype", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!w0 || !w1 || !w2 || !w3) {
+        set_error("%s: NULL output", fn);
+        return KAPPAGEN_ENULL;
+    }
+    if (!aligned_to(w0, 4) || !aligned_to(w1, 4) || !aligned_to(w2, 4) || !aligned_to(w3, 4)) {
+        set_error("%s: outputs must be 4-byte aligned", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    return dtype == KAPPAGEN_F32 ? launch_words_tile<float>(n, seed, offset, w0, w1, w2, w3, (cudaStream_t)stream)
+                                 : launch_words_tile<double>(n, seed, offset, w0, w1, w2, w3, (cudaStream_t)stream);
+}
+
+template <typename T, bool FOLD, bool U64>
+static int launch_vow_tile(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2, const uint32_t* w3,
+                           const Coef<T>& C, T* vx, T* vy, T* vz, cudaStream_t st) {
+    constexpr int threads = TileTraits<T>::threads;
+    constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
+    int grid = 0, rc;
+    if ((rc = grid_for<velocity_of_words_tile_kernel<T, FOLD, U64>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+    velocity_of_words_tile_kernel<T, FOLD, U64><<<grid, threads, 0, st>>>(n, w0, w1, w2, w3, C, vx, vy, vz);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_velocity_of_words_tile(int64_t n, const uint32_t* w0, const uint32_t* w1, const uint32_t* w2,
+                                               const uint32_t* w3, double kappa, double theta, int dtype, uint32_t flags,
+                                               void* vx, void* vy, void* vz, void* stream) {
+    const char* fn = "kappagen_velocity_of_words_tile";
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta) || (flags & ~(uint32_t)KAPPAGEN_U1_64)) {
+        set_error("%s: need finite kappa > 3/2, theta >= 0, flags in {0, KAPPAGEN_U1_64}", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    const bool u64 = (flags & KAPPAGEN_U1_64) != 0;
+    if (!w0 || !w1 || !w2 || (u64 && !w3)) {
+        set_error("%s: NULL word array", fn);
+        return KAPPAGEN_ENULL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32) {
+        const bool fold = theta_folds(theta);              // the same choice kappagen_sample makes
+        const Coef<float> C = host_coef_f32(kappa, theta, fold);
+        float *x = (float*)vx, *y = (float*)vy, *z = (float*)vz;
+        if (fold) return u64 ? launch_vow_tile<float, true, true>(n, w0, w1, w2, w3, C, x, y, z, st)
+                             : launch_vow_tile<float, true, false>(n, w0, w1, w2, w3, C, x, y, z, st);
+        return u64 ? launch_vow_tile<float, false, true>(n, w0, w1, w2, w3, C, x, y, z, st)
+                   : launch_vow_tile<float, false, false>(n, w0, w1, w2, w3, C, x, y, z, st);
+    }
+    const Coef<double> C = host_coef_f64(kappa, theta);
+    double *x = (double*)vx, *y = (double*)vy, *z = (double*)vz;
+    return u64 ? launch_vow_tile<double, false, true>(n, w0, w1, w2, w3, C, x, y, z, st)
+               : launch_vow_tile<double, false, false>(n, w0, w1, w2, w3, C, x, y, z, st);
 }
 
 // End-to-end path: host destination, chunked, double-buffered (the copy of chunk c overlaps the kernel

@@ -121,24 +121,26 @@ __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& 
     group_words<G>(g0, K, w0, w1, w2, w3);
     words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
 }
-// The same for a group known not to wrap its low counter word, given the shared head: no branch.
-template <bool FOLD, bool U64, typename T, int G>
-__device__ __forceinline__ void group_velocities_head(uint32_t lo, const PhiloxHead& H, const PhiloxKeys& K, const Coef<T>& C,
-                                                      T (&ox)[G], T (&oy)[G], T (&oz)[G]) {
-    uint32_t w0[G], w1[G], w2[G], w3[G];
+// Words of group j of a WHOLE tile (all of it inside one 2^32 block of counters): shared Philox head, no branch.
+// lo_first = lo32(counter of the thread's first particle in the tile), q_first = M0 * lo_first; group j starts
+// j * threads * G particles later.  Where TileTraits<T>::round1_add holds, round 1's product of every particle is
+// q_first plus a compile-time constant instead of a multiply.  This is the ONE function through which the
+// samplers, the histogram kernel and the kappagen_words_tile test hook draw the words of a whole tile.
+template <typename T, int G>
+__device__ __forceinline__ void tile_group_words(uint32_t lo_first, uint64_t q_first, int j, const PhiloxHead& H, const PhiloxKeys& K,
+                                                 uint32_t (&w0)[G], uint32_t (&w1)[G], uint32_t (&w2)[G], uint32_t (&w3)[G]) {
+    const uint32_t delta = (uint32_t)(j * (TileTraits<T>::threads * G));
 #pragma unroll
-    for (int e = 0; e < G; ++e) particle_words_head(lo + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
-    words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
+    for (int e = 0; e < G; ++e) {
+        if constexpr (TileTraits<T>::round1_add)
+            particle_words_q0(q_first + (uint64_t)kPhiloxM0 * (uint64_t)(delta + (uint32_t)e), H, K, w0[e], w1[e], w2[e], w3[e]);
+        else
+            particle_words_head(lo_first + delta + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
+    }
 }
-// q_first = M0 * lo32(counter of the thread's first particle in the tile); this group starts `delta` later.
-template <bool FOLD, bool U64, typename T, int G>
-__device__ __forceinline__ void group_velocities_head(uint64_t q_first, uint32_t delta, const PhiloxHead& H, const PhiloxKeys& K,
-                                                      const Coef<T>& C, T (&ox)[G], T (&oy)[G], T (&oz)[G]) {
-    uint32_t w0[G], w1[G], w2[G], w3[G];
-#pragma unroll
-    for (int e = 0; e < G; ++e)
-        particle_words_q0(q_first + (uint64_t)kPhiloxM0 * (uint64_t)(delta + (uint32_t)e), H, K, w0[e], w1[e], w2[e], w3[e]);
-    words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox, oy, oz);
+// True when the tile starting at global counter g_tile may take the whole-tile path.
+__device__ __forceinline__ bool tile_in_one_block(uint64_t g_tile, int64_t tile) {
+    return (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)tile;
 }
 
 // Streaming (evict-first) 128-bit store: the planes are never re-read by this library.
@@ -193,21 +195,19 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
     constexpr int64_t kTile = (int64_t)kT * G * NG;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (VEC && TileTraits<T>::joint && base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+        if (VEC && TileTraits<T>::joint && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             // whole tile in range and inside one 2^32 block of counters: one Philox head for the tile and all
             // groups of the thread in one straight line -- no branch between them, so their independent chains
             // interleave and share the materialised constants; stores last
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
-            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)((uint32_t)g_tile + threadIdx.x * (uint32_t)G);
+            const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
             T ox[NG][G], oy[NG][G], oz[NG][G];
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
-                if constexpr (TileTraits<T>::round1_add) {
-                    group_velocities_head<FOLD, U64>(q_first, (uint32_t)(j * (kT * G)), H, K, C, ox[j], oy[j], oz[j]);
-                } else {
-                    const uint32_t lo = (uint32_t)g_tile + (uint32_t)(j * (kT * G)) + threadIdx.x * (uint32_t)G;
-                    group_velocities_head<FOLD, U64>(lo, H, K, C, ox[j], oy[j], oz[j]);
-                }
+                uint32_t w0[G], w1[G], w2[G], w3[G];
+                tile_group_words<T, G>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
+                words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
             }
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
@@ -338,21 +338,21 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
     const bool whole_groups = ppc % (uint32_t)G == 0u;                 // every 128-bit group inside one cell
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (VEC && whole_groups && base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+        if (VEC && whole_groups && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             // whole tile in range and inside one 2^32 block of counters: the straight-line tile of the
             // uniform sampler (one Philox head; float: round-1 products by constant additions), one Coef per group
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
-            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)((uint32_t)g_tile + threadIdx.x * (uint32_t)G);
+            const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
             T ox[kGroups][G], oy[kGroups][G], oz[kGroups][G];
 #pragma unroll
             for (int j = 0; j < kGroups; ++j) {
                 const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
                 const int64_t cell0 = cell_of(i, ppc, magic);
                 const Coef<T> C = W[cell0];
-                if constexpr (TileTraits<T>::round1_add)
-                    group_velocities_head<false, false>(q_first, (uint32_t)(j * (kThreads * G)), H, K, C, ox[j], oy[j], oz[j]);
-                else
-                    group_velocities_head<false, false>((uint32_t)(offset + (uint64_t)i), H, K, C, ox[j], oy[j], oz[j]);
+                uint32_t w0[G], w1[G], w2[G], w3[G];
+                tile_group_words<T, G>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
+                words_to_velocities<false, false>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
                 if (drift != nullptr) {
                     const T* d = drift + 3 * cell0 * drift_stride;
                     const T dx = d[0], dy = d[1], dz = d[2];
@@ -461,16 +461,12 @@ __device__ __forceinline__ void group_speeds(uint64_t g0, const PhiloxKeys& K, c
 #pragma unroll
     for (int e = 0; e < 2; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
 }
-// Speeds of one group from precomputed round-1 products (whole-tile path, see sample_kernel).
-template <bool U64, bool ADD, typename T, int G>
-__device__ __forceinline__ void group_speeds_head(uint64_t q_first, uint32_t lo_first, uint32_t delta, const PhiloxHead& H,
+// Speeds of one group of a whole tile (words through tile_group_words, as in sample_kernel).
+template <bool U64, typename T, int G>
+__device__ __forceinline__ void group_speeds_tile(uint32_t lo_first, uint64_t q_first, int j, const PhiloxHead& H,
                                                   const PhiloxKeys& K, const Coef<T>& C, T (&s)[G]) {
     uint32_t w0[G], w1[G], w2[G], w3[G];
-#pragma unroll
-    for (int e = 0; e < G; ++e) {
-        if (ADD) particle_words_q0(q_first + (uint64_t)kPhiloxM0 * (uint64_t)(delta + (uint32_t)e), H, K, w0[e], w1[e], w2[e], w3[e]);
-        else particle_words_head(lo_first + delta + (uint32_t)e, H, K, w0[e], w1[e], w2[e], w3[e]);
-    }
+    tile_group_words<T, G>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
     if constexpr (sizeof(T) == 4) {
 #pragma unroll
         for (int e = 0; e < G; e += 2) up2(speed2_f32x2<U64>(w0[e], w0[e + 1], w3[e], w3[e + 1], C), s[e], s[e + 1]);
@@ -496,7 +492,7 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
     uint32_t* mine = sh_hist + ((threadIdx.x >> 5) % (unsigned)replicas) * nbins;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (base + kTile <= n && (uint32_t)g_tile <= 0xFFFFFFFFu - (uint32_t)kTile) {
+        if (base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             // whole tile in range and inside one 2^32 block of counters: straight line, one Philox head
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
@@ -504,7 +500,7 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
             T s[NG][G];
 #pragma unroll
             for (int j = 0; j < NG; ++j)
-                group_speeds_head<U64, TileTraits<T>::round1_add>(q_first, lo_first, (uint32_t)(j * (kThreads * G)), H, K, C, s[j]);
+                group_speeds_tile<U64>(lo_first, q_first, j, H, K, C, s[j]);
 #pragma unroll
             for (int j = 0; j < NG; ++j) {
 #pragma unroll
@@ -564,6 +560,87 @@ velocity_of_words_kernel(int64_t n, const uint32_t* __restrict__ w0, const uint3
         vx[i] = x;
         vy[i] = y;
         vz[i] = z;
+    }
+}
+
+// The words exactly as sample_kernel<T> draws them: the same tile walk, the same whole-tile test, on the
+// whole-tile path tile_group_words (shared head, constant-addition round 1 for float), elsewhere group_words
+// (per-group head, per-particle counters where the low word wraps).  kappagen_words_tile.
+template <typename T>
+__global__ void __launch_bounds__(TileTraits<T>::threads)
+words_tile_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,
+                  uint32_t* __restrict__ o1, uint32_t* __restrict__ o2, uint32_t* __restrict__ o3) {
+    constexpr int G = 16 / sizeof(T);
+    constexpr int NG = TileTraits<T>::groups;
+    constexpr int kT = TileTraits<T>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        const uint64_t g_tile = offset + (uint64_t)base;
+        const bool whole = base + kTile <= n && tile_in_one_block(g_tile, kTile);
+        const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
+        const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
+        const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
+#pragma unroll
+        for (int j = 0; j < NG; ++j) {
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+            uint32_t w0[G], w1[G], w2[G], w3[G];
+            if (whole) tile_group_words<T, G>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
+            else if (i < n) group_words<G>(offset + (uint64_t)i, K, w0, w1, w2, w3);
+#pragma unroll
+            for (int e = 0; e < G; ++e) {
+                if (i + e < n) {
+                    o0[i + e] = w0[e];
+                    o1[i + e] = w1[e];
+                    o2[i + e] = w2[e];
+                    o3[i + e] = w3[e];
+                }
+            }
+        }
+    }
+}
+
+// S2-S6 on caller-chosen words through the code sample_kernel<T> ships: every thread takes the NG groups of
+// a tile in one straight line through words_to_velocities (float: the packed pairs of math_f32x2.cuh; double:
+// the 2 NG interleaved chains), exactly as the whole-tile path instantiates them -- only the source of the
+// words differs (memory instead of Philox).  Past the end the last word is repeated and nothing is stored.
+// kappagen_velocity_of_words_tile.
+template <typename T, bool FOLD, bool U64>
+__global__ void __launch_bounds__(TileTraits<T>::threads, TileTraits<T>::minb)
+velocity_of_words_tile_kernel(int64_t n, const uint32_t* __restrict__ p0, const uint32_t* __restrict__ p1,
+                              const uint32_t* __restrict__ p2, const uint32_t* __restrict__ p3, const __grid_constant__ Coef<T> C,
+                              T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    constexpr int G = 16 / sizeof(T);
+    constexpr int NG = TileTraits<T>::groups;
+    constexpr int kT = TileTraits<T>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        T ox[NG][G], oy[NG][G], oz[NG][G];
+#pragma unroll
+        for (int j = 0; j < NG; ++j) {
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+            uint32_t w0[G], w1[G], w2[G], w3[G];
+#pragma unroll
+            for (int e = 0; e < G; ++e) {
+                const int64_t k = i + e < n ? i + e : n - 1;
+                w0[e] = p0[k];
+                w1[e] = p1[k];
+                w2[e] = p2[k];
+                w3[e] = U64 ? p3[k] : 0u;
+            }
+            words_to_velocities<FOLD, U64>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < NG; ++j) {
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+#pragma unroll
+            for (int e = 0; e < G; ++e) {
+                if (i + e < n) {
+                    vx[i + e] = ox[j][e];
+                    vy[i + e] = oy[j][e];
+                    vz[i + e] = oz[j][e];
+                }
+            }
+        }
     }
 }
 

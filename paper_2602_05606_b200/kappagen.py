@@ -56,13 +56,16 @@ def lib() -> ctypes.CDLL:
         L.kappagen_sample_host.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp]
         L.kappagen_baseline_mt.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp, vp]
         L.kappagen_words.argtypes = [i64, u64, u64, vp, vp, vp, vp]
+        L.kappagen_words_tile.argtypes = [i64, u64, u64, ci, vp, vp, vp, vp, vp]
+        L.kappagen_velocity_of_words_tile.argtypes = [i64, vp, vp, vp, vp, f64, f64, ci, ctypes.c_uint32, vp, vp, vp, vp]
         L.kappagen_velocity_of_words.argtypes = [i64, vp, vp, vp, f64, f64, ci, vp, vp, vp, vp]
         dp = ctypes.POINTER(ctypes.c_double)
         L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
         L.kappagen_last_error.restype = ctypes.c_char_p
         for name in ("kappagen_speed_histogram", "kappagen_relative_entropy", "kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
                      "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
-                     "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version"):
+                     "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version",
+                     "kappagen_words_tile", "kappagen_velocity_of_words_tile"):
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -101,14 +104,49 @@ def _stream(stream) -> int:
     return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
 
 
+def _dev(t, dtype, min_numel: int, what: str):
+    """A device tensor whose data_ptr() the library may use: CUDA, contiguous, of `dtype`, >= min_numel elements."""
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise ValueError("%s must be a CUDA tensor" % what)
+    if dtype is not None and t.dtype not in (dtype if isinstance(dtype, tuple) else (dtype,)):
+        raise ValueError("%s must have dtype %s, got %s" % (what, dtype, t.dtype))
+    if not t.is_contiguous() or t.numel() < min_numel:
+        raise ValueError("%s must be contiguous with >= %d elements (has %d)" % (what, min_numel, t.numel()))
+    return t
+
+
+def _same_device(*ts):
+    devs = {t.device for t in ts if t is not None}
+    if len(devs) > 1:
+        raise ValueError("all tensors of one call must live on the same device, got %s" % sorted(map(str, devs)))
+
+
 def _planes(n: int, code: int, out, device):
     if out is None:
         return tuple(torch.empty(n, dtype=_torch_dtype(code), device=device) for _ in range(3))
     vx, vy, vz = out
     for t in (vx, vy, vz):
-        if t.dtype != _torch_dtype(code) or t.numel() < n or not t.is_contiguous():
-            raise ValueError("output planes must be contiguous, of the requested dtype, with >= n elements")
+        _dev(t, _torch_dtype(code), n, "output plane")
+    _same_device(vx, vy, vz)
     return vx, vy, vz
+
+
+def _cell_inputs(ppc: int, kappa, theta, drift, drift_stride: int):
+    """Checks shared by sample_cells / sample_cells_moments / load_cells_record; returns (code, ncell)."""
+    code = _dtype_code(kappa.dtype)
+    ncell = kappa.numel()
+    _dev(kappa, None, ncell, "kappa")
+    _dev(theta, kappa.dtype, ncell, "theta")
+    if theta.numel() != ncell:
+        raise ValueError("kappa and theta must have the same length")
+    if drift_stride not in (0, 1):
+        raise ValueError("drift_stride must be 0 (one shared vector) or 1 (per cell)")
+    if drift is not None:
+        _dev(drift, kappa.dtype, 3 if drift_stride == 0 else 3 * ncell, "drift")
+    _same_device(kappa, theta, drift)
+    if ppc < 0:
+        raise ValueError("ppc must be >= 0")
+    return code, ncell
 
 
 def params(kappa: float):
@@ -145,14 +183,13 @@ def cells_workspace_bytes(ncell: int, dtype="f32") -> int:
 def sample_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0,
                  seed: int = 0, offset: int = 0, out=None, workspace=None, stream=None):
     """kappagen_sample_cells: kappa, theta (and drift) are device tensors of the output dtype."""
-    code = _dtype_code(kappa.dtype)
-    ncell = kappa.numel()
-    if theta.dtype != kappa.dtype or theta.numel() != ncell or (drift is not None and drift.dtype != kappa.dtype):
-        raise ValueError("kappa, theta and drift must share dtype; kappa and theta must share length")
+    code, ncell = _cell_inputs(ppc, kappa, theta, drift, drift_stride)
     vx, vy, vz = _planes(ncell * ppc, code, out, kappa.device)
+    _same_device(kappa, vx)
     need = cells_workspace_bytes(ncell, code)
     if workspace is None:
         workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    _dev(workspace, None, 0, "workspace")
     _check(lib().kappagen_sample_cells(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
                                        drift.data_ptr() if drift is not None else None, drift_stride, seed, offset,
                                        code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), workspace.data_ptr(),
@@ -165,16 +202,16 @@ def sample_cells_moments(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, dri
                          store: bool = True):
     """kappagen_sample_cells_moments: returns ((vx, vy, vz) or None, moments[ncell, 4]).  store=False passes
     NULL planes: moments only, no velocity reaches HBM."""
-    code = _dtype_code(kappa.dtype)
-    ncell = kappa.numel()
-    if theta.dtype != kappa.dtype or theta.numel() != ncell or (drift is not None and drift.dtype != kappa.dtype):
-        raise ValueError("kappa, theta and drift must share dtype; kappa and theta must share length")
+    code, ncell = _cell_inputs(ppc, kappa, theta, drift, drift_stride)
     planes = _planes(ncell * ppc, code, out, kappa.device) if store else None
     if moments is None:
         moments = torch.empty((ncell, 4), dtype=kappa.dtype, device=kappa.device)
+    _dev(moments, kappa.dtype, 4 * ncell, "moments")
     need = cells_workspace_bytes(ncell, code)
     if workspace is None:
         workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    _dev(workspace, None, 0, "workspace")
+    _same_device(kappa, moments, workspace, *(planes or ()))
     ptrs = [p.data_ptr() for p in planes] if store else [None, None, None]
     _check(lib().kappagen_sample_cells_moments(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
                                                drift.data_ptr() if drift is not None else None, drift_stride, seed,
@@ -203,8 +240,8 @@ def baseline_mt(n: int, kappa: float, theta: float, seed: int, offset: int = 0, 
     """kappagen_baseline_mt: the rejection-based comparison generator (exact Kappa distribution)."""
     code = _dtype_code(dtype)
     vx, vy, vz = _planes(n, code, out, device)
-    if trip_counters is not None and (trip_counters.dtype not in (torch.int64, torch.uint64) or trip_counters.numel() < 2):
-        raise ValueError("trip_counters must be a device tensor of two 64-bit integers")
+    if trip_counters is not None:
+        _dev(trip_counters, (torch.int64, torch.uint64), 2, "trip_counters")
     _check(lib().kappagen_baseline_mt(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
                                       _stream(stream), trip_counters.data_ptr() if trip_counters is not None else None))
     return vx, vy, vz
@@ -230,8 +267,9 @@ def velocity_of_words_u64(w0, w1, w2, w3, kappa: float, theta: float, dtype="f32
     code = _dtype_code(dtype)
     n = w0.numel()
     for w in (w0, w1, w2, w3):
-        if w.dtype != torch.int32 or w.numel() != n or not w.is_contiguous():
-            raise ValueError("words must be contiguous int32 tensors of equal length")
+        _dev(w, torch.int32, n, "words")
+        if w.numel() != n:
+            raise ValueError("words must have equal length")
     vx, vy, vz = _planes(n, code, None, w0.device)
     _check(lib().kappagen_velocity_of_words_u64(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(), w3.data_ptr(), kappa,
                                                 theta, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
@@ -243,11 +281,34 @@ def velocity_of_words(w0, w1, w2, kappa: float, theta: float, dtype="f32", strea
     code = _dtype_code(dtype)
     n = w0.numel()
     for w in (w0, w1, w2):
-        if w.dtype != torch.int32 or w.numel() != n or not w.is_contiguous():
-            raise ValueError("words must be contiguous int32 tensors of equal length")
+        _dev(w, torch.int32, n, "words")
+        if w.numel() != n:
+            raise ValueError("words must have equal length")
     vx, vy, vz = _planes(n, code, None, w0.device)
     _check(lib().kappagen_velocity_of_words(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(), kappa, theta, code,
                                             vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
+    return vx, vy, vz
+
+def words_tile(n: int, seed: int, offset: int = 0, dtype="f32", stream=None, device="cuda"):
+    """kappagen_words_tile: all four words, drawn through the tile path of kappagen_sample's kernel for `dtype`."""
+    w = tuple(torch.empty(n, dtype=torch.int32, device=device) for _ in range(4))
+    _check(lib().kappagen_words_tile(n, seed, offset, _dtype_code(dtype), w[0].data_ptr(), w[1].data_ptr(), w[2].data_ptr(),
+                                     w[3].data_ptr(), _stream(stream)))
+    return w
+
+
+def velocity_of_words_tile(w0, w1, w2, kappa: float, theta: float, dtype="f32", w3=None, flags: int = 0, stream=None):
+    """kappagen_velocity_of_words_tile: S2-S6 on caller-chosen words through the shipped straight-line tile body."""
+    code = _dtype_code(dtype)
+    n = w0.numel()
+    for w in (w0, w1, w2) + ((w3,) if w3 is not None else ()):
+        _dev(w, torch.int32, n, "words")
+        if w.numel() != n:
+            raise ValueError("words must have equal length")
+    vx, vy, vz = _planes(n, code, None, w0.device)
+    _check(lib().kappagen_velocity_of_words_tile(n, w0.data_ptr(), w1.data_ptr(), w2.data_ptr(),
+                                                 w3.data_ptr() if w3 is not None else None, kappa, theta, code, flags,
+                                                 vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
     return vx, vy, vz
 
 
@@ -257,6 +318,7 @@ def speed_histogram(n: int, kappa: float, seed: int, offset: int = 0, dtype="f32
     unsigned 64-bit counters, zeroed here when not given)."""
     if hist is None:
         hist = torch.zeros(nbins, dtype=torch.int64, device=device)
+    _dev(hist, (torch.int64, torch.uint64), nbins, "hist")
     _check(lib().kappagen_speed_histogram(n, kappa, seed, offset, _dtype_code(dtype), flags, dv, nbins, hist.data_ptr(),
                                           _stream(stream)))
     return hist

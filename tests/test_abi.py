@@ -27,7 +27,7 @@ def declared_symbols():
 
 def test_every_declared_symbol_is_exported(L):
     names = declared_symbols()
-    assert len(names) == 16 and "kappagen_speed_histogram" in names and "kappagen_sample_flags" in names and "kappagen_sample_cells_moments" in names and "kappagen_sample" in names and "kappagen_sample_cells" in names
+    assert len(names) >= 18 and "kappagen_words_tile" in names and "kappagen_velocity_of_words_tile" in names and "kappagen_speed_histogram" in names and "kappagen_sample_flags" in names and "kappagen_sample_cells_moments" in names and "kappagen_sample" in names and "kappagen_sample_cells" in names
     for name in names:
         assert getattr(L, name) is not None
 
