@@ -87,18 +87,18 @@ def fits_f32():
 
 
 def fits_f64():
-    # ln(m) = 2 f P(f^2), f = (m-1)/(m+1), m in [sqrt(1/2), sqrt(2)] -> f^2 <= ((sqrt2-1)/(sqrt2+1))^2
-    zmax = ((mp.sqrt(2) - 1) / (mp.sqrt(2) + 1)) ** 2
-    for deg in (6,):
-        report("P(z) = atanh(sqrt z)/sqrt z", lambda z: mp.atanh(mp.sqrt(z)) / mp.sqrt(z) if z > TINY else mp.mpf(1),
-               0, zmax * (1 + mp.mpf(1) / 1000), deg, r64, hex64)
+    # ln(m) = 2 f P(f^2), f = (m-1)/(m+1).  k = round(log2 S) is taken from the high words of numerator and
+    # denominator (a piecewise-linear log2, off by < 0.09), so m = S 2^-k lies in [2^-0.59, 2^0.59].
+    m = mp.power(2, mp.mpf("0.59"))
+    zmax = ((m - 1) / (m + 1)) ** 2
+    report("P(z) = atanh(sqrt z)/sqrt z", lambda z: mp.atanh(mp.sqrt(z)) / mp.sqrt(z) if z > TINY else mp.mpf(1),
+           0, zmax, 5, r64, hex64)
     # expm1(rho) = rho Q(rho), |rho| <= ln2/2
     h = mp.log(2) / 2 * (1 + mp.mpf(1) / 1000)
-    for deg in (8,):
-        report("Q(rho) = expm1(rho)/rho", lambda r: mp.expm1(r) / r if abs(r) > TINY else mp.mpf(1), -h, h, deg, r64, hex64)
+    report("Q(rho) = expm1(rho)/rho", lambda r: mp.expm1(r) / r if abs(r) > TINY else mp.mpf(1), -h, h, 8, r64, hex64)
     report("sin(pi q/2)/q in z = q^2", lambda z: mp.sin(mp.pi / 2 * mp.sqrt(z)) / mp.sqrt(z) if z > TINY else mp.pi / 2,
            0, 0.25, 5, r64, hex64)
-    report("cos(pi q/2) in z = q^2", lambda z: mp.cos(mp.pi / 2 * mp.sqrt(z)), 0, 0.25, 6, r64, hex64)
+    report("cos(pi q/2) in z = q^2", lambda z: mp.cos(mp.pi / 2 * mp.sqrt(z)), 0, 0.25, 5, r64, hex64)
 
 
 if __name__ == "__main__":

@@ -332,27 +332,28 @@ static int words_impl(const char* fn, int64_t n, uint64_t seed, uint64_t offset,
 template <typename T, bool U64>
 static int launch_hist(int64_t n, uint64_t offset, const PhiloxKeys& K, const Coef<T>& C, T inv, int nbins,
                        unsigned long long* hist, cudaStream_t st) {
-    static_assert(TileTraits<T>::threads == kThreads, "the histogram kernel uses kThreads per block");
-    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * TileTraits<T>::groups;
-    int replicas = (48 * 1024) / (nbins * 4);
-    if (replicas > kThreads / 32) replicas = kThreads / 32;
+    constexpr int threads = TileTraits<T>::threads;                  // the sample kernel's block and tile shape
+    constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
+    constexpr int warps = threads / 32;
+    int replicas = (40 * 1024) / (nbins * 4);                        // (+ the double chain's tables: static shared memory)
+    if (replicas > warps) replicas = warps;
     if (replicas < 1) replicas = 1;
     const size_t smem = (size_t)replicas * nbins * 4;
     int grid = 0, rc;
     // The block counts into 32-bit shared-memory replicas and flushes them once at its end.  A replica sees the
-    // particles of ceil(warps/replicas) of the block's 8 warps, so per launch a block may process at most
+    // particles of ceil(warps/replicas) of the block's warps, so per launch a block may process at most
     // 2^32 / that share of its particles: split larger calls into launches of `cap` particles (whatever the
     // device's SM count or the occupancy), each flushing into the caller's 64-bit counters.
     const int64_t tiles_all = (n + tile - 1) / tile;
-    if ((rc = grid_for<speed_histogram_kernel<T, U64>>(tiles_all, &grid, kThreads, smem)) != KAPPAGEN_OK) return rc;
-    const int warps = kThreads / 32, share = (warps + replicas - 1) / replicas;
+    if ((rc = grid_for<speed_histogram_kernel<T, U64>>(tiles_all, &grid, threads, smem)) != KAPPAGEN_OK) return rc;
+    const int share = (warps + replicas - 1) / replicas;
     const int64_t per_block = (((int64_t)1 << 32) - 1) / share * warps / tile * tile;     // particles, whole tiles
     const int64_t cap = per_block * (int64_t)(grid < 1 ? 1 : grid) / 2;                   // factor 2: uneven tile counts per block
     for (int64_t done = 0; done < n;) {
         const int64_t m = (n - done) < cap ? (n - done) : cap;
         int g = 0;
-        if ((rc = grid_for<speed_histogram_kernel<T, U64>>((m + tile - 1) / tile, &g, kThreads, smem)) != KAPPAGEN_OK) return rc;
-        speed_histogram_kernel<T, U64><<<g, kThreads, smem, st>>>(m, offset + (uint64_t)done, K, C, inv, nbins, replicas, hist);
+        if ((rc = grid_for<speed_histogram_kernel<T, U64>>((m + tile - 1) / tile, &g, threads, smem)) != KAPPAGEN_OK) return rc;
+        speed_histogram_kernel<T, U64><<<g, threads, smem, st>>>(m, offset + (uint64_t)done, K, C, inv, nbins, replicas, hist);
         KG_CUDA(cudaGetLastError());
         done += m;
     }

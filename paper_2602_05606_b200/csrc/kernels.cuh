@@ -36,7 +36,7 @@ constexpr int kGroups = 2;  // 128-bit groups per thread per tile
 #define KG_F64_MINB 1
 #endif
 #ifndef KG_F64_THREADS
-#define KG_F64_THREADS 256
+#define KG_F64_THREADS 384
 #endif
 #ifndef KG_JOINT_F32
 #define KG_JOINT_F32 1
@@ -57,6 +57,12 @@ template <typename T> struct TileTraits {
     // bound (float: +1 %), costs where it is not (double: -5 %).
     static constexpr bool round1_add = sizeof(T) == 4;
 };
+
+// Shared-memory lookup tables of the double chain (math_f64.cuh); nothing for float.  Called once per block, by all
+// its threads, before the first particle.
+template <typename T> __device__ __forceinline__ void math_tables_init() {
+    if constexpr (sizeof(T) == 8) f64_tables_init();
+}
 
 template <typename T> struct Vec128;
 template <> struct Vec128<float> { using type = float4; };
@@ -126,10 +132,10 @@ __device__ __forceinline__ void group_velocities(uint64_t g0, const PhiloxKeys& 
 // j * threads * G particles later.  Where TileTraits<T>::round1_add holds, round 1's product of every particle is
 // q_first plus a compile-time constant instead of a multiply.  This is the ONE function through which the
 // samplers, the histogram kernel and the kappagen_words_tile test hook draw the words of a whole tile.
-template <typename T, int G>
+template <typename T, int G, int THREADS = TileTraits<T>::threads>
 __device__ __forceinline__ void tile_group_words(uint32_t lo_first, uint64_t q_first, int j, const PhiloxHead& H, const PhiloxKeys& K,
                                                  uint32_t (&w0)[G], uint32_t (&w1)[G], uint32_t (&w2)[G], uint32_t (&w3)[G]) {
-    const uint32_t delta = (uint32_t)(j * (TileTraits<T>::threads * G));
+    const uint32_t delta = (uint32_t)(j * (THREADS * G));                   // THREADS = the calling kernel's block size
 #pragma unroll
     for (int e = 0; e < G; ++e) {
         if constexpr (TileTraits<T>::round1_add)
@@ -193,6 +199,7 @@ sample_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, 
     constexpr int NG = TileTraits<T>::groups;
     constexpr int kT = TileTraits<T>::threads;
     constexpr int64_t kTile = (int64_t)kT * G * NG;
+    math_tables_init<T>();
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         const uint64_t g_tile = offset + (uint64_t)base;
         if (VEC && TileTraits<T>::joint && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
@@ -336,6 +343,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
     constexpr int G = 16 / sizeof(T);
     constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
     const bool whole_groups = ppc % (uint32_t)G == 0u;                 // every 128-bit group inside one cell
+    math_tables_init<T>();
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         const uint64_t g_tile = offset + (uint64_t)base;
         if (VEC && whole_groups && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
@@ -351,7 +359,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                 const int64_t cell0 = cell_of(i, ppc, magic);
                 const Coef<T> C = W[cell0];
                 uint32_t w0[G], w1[G], w2[G], w3[G];
-                tile_group_words<T, G>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
+                tile_group_words<T, G, kThreads>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
                 words_to_velocities<false, false>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
                 if (drift != nullptr) {
                     const T* d = drift + 3 * cell0 * drift_stride;
@@ -480,14 +488,16 @@ __device__ __forceinline__ int bin_of(double s, double inv) { return __double2in
 
 // inv = 1/dv (double) or 1/(2 dv) (float, whose chain returns 2V), rounded to T.
 template <typename T, bool U64>
-__global__ void __launch_bounds__(kThreads, TileTraits<T>::minb)
+__global__ void __launch_bounds__(TileTraits<T>::threads, TileTraits<T>::minb)
 speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, const __grid_constant__ Coef<T> C,
                        T inv, int nbins, int replicas, unsigned long long* __restrict__ hist) {
     extern __shared__ uint32_t sh_hist[];
     constexpr int G = 16 / sizeof(T);
     constexpr int NG = TileTraits<T>::groups;            // the sample kernel's tile shape: same chains, same trade-off
-    constexpr int64_t kTile = (int64_t)kThreads * G * NG;
-    for (int b = threadIdx.x; b < nbins * replicas; b += kThreads) sh_hist[b] = 0u;
+    constexpr int kT = TileTraits<T>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
+    for (int b = threadIdx.x; b < nbins * replicas; b += kT) sh_hist[b] = 0u;
+    math_tables_init<T>();
     __syncthreads();
     uint32_t* mine = sh_hist + ((threadIdx.x >> 5) % (unsigned)replicas) * nbins;
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
@@ -510,7 +520,7 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
         }
 #pragma unroll
         for (int j = 0; j < NG; ++j) {
-            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
             if (i < n) {
                 T s[G];
                 group_speeds<U64>(offset + (uint64_t)i, K, C, s);
@@ -522,7 +532,7 @@ speed_histogram_kernel(int64_t n, uint64_t offset, const __grid_constant__ Philo
         }
     }
     __syncthreads();
-    for (int b = threadIdx.x; b < nbins; b += kThreads) {
+    for (int b = threadIdx.x; b < nbins; b += kT) {
         unsigned long long c = 0ull;
         for (int r = 0; r < replicas; ++r) c += sh_hist[r * nbins + b];
         if (c != 0ull) atomicAdd(hist + b, c);
@@ -554,6 +564,7 @@ __global__ void __launch_bounds__(kThreads)
 velocity_of_words_kernel(int64_t n, const uint32_t* __restrict__ w0, const uint32_t* __restrict__ w1,
                          const uint32_t* __restrict__ w2, const uint32_t* __restrict__ w3, const __grid_constant__ Coef<T> C,
                          T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz) {
+    math_tables_init<T>();
     for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
         T x, y, z;
         velocity<FOLD, U64>(w0[i], w1[i], w2[i], U64 ? w3[i] : 0u, C, x, y, z);
@@ -613,6 +624,7 @@ velocity_of_words_tile_kernel(int64_t n, const uint32_t* __restrict__ p0, const 
     constexpr int NG = TileTraits<T>::groups;
     constexpr int kT = TileTraits<T>::threads;
     constexpr int64_t kTile = (int64_t)kT * G * NG;
+    math_tables_init<T>();
     for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
         T ox[NG][G], oy[NG][G], oz[NG][G];
 #pragma unroll
