@@ -52,6 +52,23 @@ struct alignas(16) Coef<float> {
     float theta;  // theta, or 1 when folded
 };
 
+// Workspace record of one cell (kappagen_sample_cells): the constants of the per-particle chain -- the two that the
+// chain uses negated stored negated -- and the cell's drift: 12 values, 48 bytes (float) / 96 bytes (double), written
+// once by the pre-kernel and read once per 128-bit particle group, so that the sampling kernel has neither a drift
+// pointer nor a drift branch.
+template <typename T> struct CellRec;
+template <>
+struct alignas(16) CellRec<float> {
+    float s, ms, a, mck;       // 1/kappa*, -1/kappa*, a, -c kappa*
+    float bk4, k2, b2, th4;    // as Coef<float>, never folded
+    float theta, dx, dy, dz;   // theta (NaN marks an invalid cell), drift
+};
+template <>
+struct alignas(16) CellRec<double> {
+    Coef<double> C;
+    double dx, dy, dz, pad;
+};
+
 #ifdef __CUDACC__
 #define KAPPAGEN_HD __host__ __device__
 #else
@@ -121,6 +138,19 @@ KAPPAGEN_HD inline Coef<float> make_coef_f32(const TableIParams<F>& P, F theta, 
     C.theta = fold ? 1.0f : (float)theta;
     return C;
 }
+
+KAPPAGEN_HD inline CellRec<float> make_cell_rec(const Coef<float>& C, float dx, float dy, float dz) {
+    return CellRec<float>{C.s, -C.s, C.a, -C.ck, C.bk4, C.k2, C.b2, C.th4, C.theta, dx, dy, dz};
+}
+KAPPAGEN_HD inline CellRec<double> make_cell_rec(const Coef<double>& C, double dx, double dy, double dz) {
+    return CellRec<double>{C, dx, dy, dz, 0.0};
+}
+KAPPAGEN_HD inline Coef<float> coef_of(const CellRec<float>& R) {
+    Coef<float> C;
+    C.s = R.s; C.a = R.a; C.ck = -R.mck; C.bk4 = R.bk4; C.k2 = R.k2; C.b2 = R.b2; C.th4 = R.th4; C.theta = R.theta;
+    return C;
+}
+KAPPAGEN_HD inline Coef<double> coef_of(const CellRec<double>& R) { return R.C; }
 
 KAPPAGEN_HD inline bool theta_folds(double theta) { return theta >= 0x1p-30 && theta <= 0x1p+30; }
 

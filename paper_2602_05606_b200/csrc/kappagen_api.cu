@@ -132,14 +132,13 @@ static int sample_on_stream(const char* fn, int64_t n, double kappa, double thet
 }
 
 template <typename T, bool VEC, bool STORE, bool MOM>
-static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint64_t offset, const PhiloxKeys& K, const Coef<T>* W,
-                           const T* drift, int64_t drift_stride, T* vx, T* vy, T* vz, T* mom, int mode, int lanes,
-                           cudaStream_t st) {
+static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint32_t magic32, uint64_t offset, const PhiloxKeys& K,
+                           const CellRec<T>* W, T* vx, T* vy, T* vz, T* mom, int mode, int lanes, cudaStream_t st) {
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
     int grid = 0, rc;
     if ((rc = grid_for<sample_cells_kernel<T, VEC, STORE, MOM>>((n + tile - 1) / tile, &grid)) != KAPPAGEN_OK) return rc;
-    sample_cells_kernel<T, VEC, STORE, MOM><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, offset, K, W, drift, drift_stride,
-                                                                      vx, vy, vz, mom, mode, lanes);
+    sample_cells_kernel<T, VEC, STORE, MOM><<<grid, kThreads, 0, st>>>(n, (uint32_t)ppc, magic, magic32, offset, K, W, vx, vy, vz,
+                                                                      mom, mode, lanes);
     KG_CUDA(cudaGetLastError());
     return KAPPAGEN_OK;
 }
@@ -148,8 +147,9 @@ static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint64_t offs
 template <typename T>
 static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift,
                         int64_t drift_stride, uint64_t offset, const PhiloxKeys& K, bool vec, bool store, T* vx, T* vy,
-                        T* vz, T* mom, Coef<T>* W, cudaStream_t st) {
+                        T* vz, T* mom, CellRec<T>* W, cudaStream_t st) {
     constexpr int G = 16 / sizeof(T);
+    constexpr int64_t tile = (int64_t)kThreads * G * kGroups;
     int mode = kMomNone, lanes = 1;
     if (mom != nullptr) {
         const int L = ppc / G;
@@ -158,7 +158,7 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
         else mode = kMomAtomic;
     }
     const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
-    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, W,
+    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, drift, drift_stride, W,
                                                               (mode == kMomWarp || mode == kMomAtomic) ? mom : nullptr);
     KG_CUDA(cudaGetLastError());
     const int64_t n = ncell * (int64_t)ppc;
@@ -172,7 +172,10 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
     } else if ((uint64_t)n <= (~0ull) / up) {
         magic = (~0ull) / up + 1;                           // >= 2^32 > 64 for every ppc < 2^31
     }
-#define KG_CELLS(V, S, M) launch_cells_as<T, V, S, M>(n, ppc, magic, offset, K, W, drift, drift_stride, vx, vy, vz, mom, mode, lanes, st)
+    // inside a tile: floor(o/ppc) = mulhi32(o, ceil(2^32/ppc)), exact while o * ppc < 2^32 (o < tile + ppc); 0 = not used
+    uint32_t magic32 = 0;
+    if (up >= 2 && ((uint64_t)tile + up) * up < (1ull << 32)) magic32 = (uint32_t)(((1ull << 32) + up - 1) / up);
+#define KG_CELLS(V, S, M) launch_cells_as<T, V, S, M>(n, ppc, magic, magic32, offset, K, W, vx, vy, vz, mom, mode, lanes, st)
     if (mom == nullptr) return vec ? KG_CELLS(true, true, false) : KG_CELLS(false, true, false);
     if (!store) return KG_CELLS(true, false, true);
     return vec ? KG_CELLS(true, true, true) : KG_CELLS(false, true, true);
@@ -211,7 +214,7 @@ extern "C" int kappagen_sample_flags(int64_t n, double kappa, double theta, uint
 
 extern "C" size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype) {
     if (ncell <= 0 || (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64)) return 0;
-    return (size_t)ncell * (dtype == KAPPAGEN_F32 ? sizeof(Coef<float>) : sizeof(Coef<double>));
+    return (size_t)ncell * (dtype == KAPPAGEN_F32 ? sizeof(CellRec<float>) : sizeof(CellRec<double>));
 }
 
 static int cells_impl(const char* fn, int64_t ncell, int32_t ppc, const void* kappa, const void* theta, const void* drift,
@@ -267,10 +270,10 @@ static int cells_impl(const char* fn, int64_t ncell, int32_t ppc, const void* ka
     if (dtype == KAPPAGEN_F32)
         return launch_cells<float>(ncell, ppc, (const float*)kappa, (const float*)theta, (const float*)drift, drift_stride,
                                    offset, K, vec, store, (float*)vx, (float*)vy, (float*)vz, (float*)moments,
-                                   (Coef<float>*)workspace, st);
+                                   (CellRec<float>*)workspace, st);
     return launch_cells<double>(ncell, ppc, (const double*)kappa, (const double*)theta, (const double*)drift, drift_stride,
                                 offset, K, vec, store, (double*)vx, (double*)vy, (double*)vz, (double*)moments,
-                                (Coef<double>*)workspace, st);
+                                (CellRec<double>*)workspace, st);
 }
 
 extern "C" int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,

@@ -244,11 +244,11 @@ template <> __device__ __forceinline__ Coef<double> cell_coef<double>(const Tabl
     return make_coef_f64<double>(P, theta);
 }
 
-// Pre-kernel: Table I lines 1-4 per cell, in double, into the workspace (one Coef<T> per cell).
+// Pre-kernel: Table I lines 1-4 per cell, in double, and the cell's drift, into the workspace (one CellRec<T> per cell).
 template <typename T>
 __global__ void __launch_bounds__(kThreads)
-cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict__ theta, Coef<T>* __restrict__ W,
-                 T* __restrict__ mom_to_zero) {
+cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict__ theta, const T* __restrict__ drift,
+                 int64_t drift_stride, CellRec<T>* __restrict__ W, T* __restrict__ mom_to_zero) {
     const int64_t cell = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (cell >= ncell) return;
     if (mom_to_zero != nullptr) {                                      // atomic moment modes accumulate into zeros
@@ -262,7 +262,12 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
     const TableIParams<double> P = table1_params<double>(ok ? kap : 2.5, lnB, c_approx_f64(ok ? kap : 2.5));
     Coef<T> C = cell_coef<T>(P, th);
     if (!ok) C.theta = (T)nan("");                                    // whole cell becomes NaN
-    W[cell] = C;
+    T dx = T(0), dy = T(0), dz = T(0);
+    if (drift != nullptr) {
+        const T* d = drift + 3 * cell * drift_stride;
+        dx = d[0]; dy = d[1]; dz = d[2];
+    }
+    W[cell] = make_cell_rec(C, dx, dy, dz);
 }
 
 // floor(i / ppc) without a 64-bit division.  magic < 64: ppc = 2^magic, a shift.  Otherwise magic =
@@ -271,13 +276,6 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
 __device__ __forceinline__ int64_t cell_of(int64_t i, uint32_t ppc, uint64_t magic) {
     if (magic < 64ull) return i >> (int)magic;
     return magic != ~0ull ? (int64_t)__umul64hi((uint64_t)i, magic) : i / (int64_t)ppc;
-}
-
-template <typename T>
-__device__ __forceinline__ void add_drift(const T* __restrict__ d, T& x, T& y, T& z) {
-    x += d[0];
-    y += d[1];
-    z += d[2];
 }
 
 // How the fused moments (kappagen_sample_cells_moments) leave the kernel.  All sums are in T.
@@ -289,14 +287,16 @@ __device__ __forceinline__ void add_drift(const T* __restrict__ d, T& x, T& y, T
 //   kMomAtomic : any ppc: per group (or per particle where a group straddles two cells) atomicAdd.
 enum MomMode : int { kMomNone = 0, kMomDirect = 1, kMomWarp = 2, kMomAtomic = 3 };
 
+// mask: the lanes that take part.  Whole tiles: every lane of the warp; the guarded path hands in the ballot of
+// its own condition (with n = ncell * ppc a cell's lanes are in range together, so the shuffle modes only ever
+// see full segments).
 template <typename T>
-__device__ __forceinline__ void moments_out(T (&ps)[4], int64_t cell, int mode, int lanes, T* __restrict__ mom) {
+__device__ __forceinline__ void moments_out(T (&ps)[4], int64_t cell, int mode, int lanes, T* __restrict__ mom, unsigned mask) {
     if (mode == kMomAtomic) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) atomicAdd(mom + 4 * cell + q, ps[q]);
         return;
     }
-    const unsigned mask = __activemask();
     const unsigned lane = threadIdx.x & (unsigned)(lanes - 1);         // lane inside the cell's segment
     if (lanes >= 4) {
         // Transposing butterfly: after two exchange steps each lane of a quad owns ONE of the four sums over
@@ -327,60 +327,120 @@ __device__ __forceinline__ void moments_out(T (&ps)[4], int64_t cell, int mode, 
         }
     }
 }
+template <typename T, int G>
+__device__ __forceinline__ void group_moments(const T (&ox)[G], const T (&oy)[G], const T (&oz)[G], T (&ps)[4]) {
+    ps[0] = ps[1] = ps[2] = ps[3] = T(0);
+#pragma unroll
+    for (int e = 0; e < G; ++e) {
+        ps[0] += ox[e];
+        ps[1] += oy[e];
+        ps[2] += oz[e];
+        ps[3] = fma(ox[e], ox[e], fma(oy[e], oy[e], fma(oz[e], oz[e], ps[3])));
+    }
+}
+
+// One cell's record through the read-only path: 128-bit loads (16 lanes of a warp share a cell at ppc = 64, so a
+// warp instruction touches a handful of sectors, resident in L1/L2).
+template <typename T> struct RecRegs;
+template <> struct RecRegs<float> { float4 q[3]; };
+template <> struct RecRegs<double> { ulonglong2 q[6]; };
+__device__ __forceinline__ void load_rec(const CellRec<float>* __restrict__ W, int64_t cell, RecRegs<float>& r) {
+    const float4* src = reinterpret_cast<const float4*>(W + cell);
+#pragma unroll
+    for (int u = 0; u < 3; ++u) r.q[u] = __ldg(src + u);
+}
+__device__ __forceinline__ void load_rec(const CellRec<double>* __restrict__ W, int64_t cell, RecRegs<double>& r) {
+    const ulonglong2* src = reinterpret_cast<const ulonglong2*>(W + cell);
+#pragma unroll
+    for (int u = 0; u < 6; ++u) r.q[u] = __ldg(src + u);
+}
+// Velocities of one 128-bit group with per-cell constants and drift, from the cell's record.  The drift enters
+// through the last multiply-add of the chain (velocity_f32 / velocity_f64, DRIFT), the same in every path.
+__device__ __forceinline__ void rec_velocities(const uint32_t (&w0)[4], const uint32_t (&w1)[4], const uint32_t (&w2)[4],
+                                               const RecRegs<float>& r, float (&ox)[4], float (&oy)[4], float (&oz)[4]) {
+    const float4 q0 = r.q[0], q1 = r.q[1], q2 = r.q[2];                  // the order of CellRec<float>
+    const Coef2 C{splat2(q0.x), splat2(q0.y), splat2(q0.z), splat2(q0.w), splat2(q1.x), splat2(q1.y), splat2(q1.z),
+                  splat2(q1.w), splat2(q2.x)};
+    const f32x2 dx = splat2(q2.y), dy = splat2(q2.z), dz = splat2(q2.w);
+#pragma unroll
+    for (int e = 0; e < 4; e += 2) {
+        const uint32_t p0[2] = {w0[e], w0[e + 1]}, p1[2] = {w1[e], w1[e + 1]}, p2[2] = {w2[e], w2[e + 1]}, p3[2] = {0u, 0u};
+        float a[2], b[2], c[2];
+        velocity_pair_f32<false, false, true>(p0, p1, p2, p3, C, a, b, c, dx, dy, dz);
+        ox[e] = a[0]; ox[e + 1] = a[1];
+        oy[e] = b[0]; oy[e + 1] = b[1];
+        oz[e] = c[0]; oz[e + 1] = c[1];
+    }
+}
+__device__ __forceinline__ double as_f64(unsigned long long b) { return __longlong_as_double((long long)b); }
+__device__ __forceinline__ void rec_velocities(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
+                                               const RecRegs<double>& r, double (&ox)[2], double (&oy)[2], double (&oz)[2]) {
+    const ulonglong2 (&q)[6] = r.q;
+    Coef<double> C;                                                    // the order of CellRec<double>
+    C.s = as_f64(q[0].x); C.a = as_f64(q[0].y); C.ck = as_f64(q[1].x); C.bk4 = as_f64(q[1].y);
+    C.k2 = as_f64(q[2].x); C.b2 = as_f64(q[2].y); C.theta = as_f64(q[3].x); C.pad = 0.0;
+#pragma unroll
+    for (int e = 0; e < 2; ++e)
+        velocity_f64<false, true>(w0[e], w1[e], w2[e], 0u, C, ox[e], oy[e], oz[e], as_f64(q[4].x), as_f64(q[4].y), as_f64(q[5].x));
+}
+// one particle (a group that straddles two cells): the scalar chain, bit-identical to the packed one
+__device__ __forceinline__ void rec_velocity(uint32_t w0, uint32_t w1, uint32_t w2, const CellRec<float>& R, float& x, float& y, float& z) {
+    velocity_f32<false, false, true>(w0, w1, w2, 0u, coef_of(R), x, y, z, R.dx, R.dy, R.dz);
+}
+__device__ __forceinline__ void rec_velocity(uint32_t w0, uint32_t w1, uint32_t w2, const CellRec<double>& R, double& x, double& y, double& z) {
+    velocity_f64<false, true>(w0, w1, w2, 0u, R.C, x, y, z, R.dx, R.dy, R.dz);
+}
 
 // Particle g = cell * ppc + j (cell-major).  A 128-bit group of G particles that lies inside one cell -- every
-// group when ppc is a multiple of G -- loads that cell's Coef<T> once and runs the same packed / shared-head
+// group when ppc is a multiple of G -- reads that cell's record once and runs the same packed / shared-head
 // code as the uniform sampler; a group that straddles a cell boundary takes the per-particle path.
+// Whole tiles (in range, inside one 2^32 block of counters) run in one straight line, as in the uniform sampler;
+// a group finds its cell with one 32-bit multiply-high from its offset inside the tile (magic32 = ceil(2^32 / ppc),
+// exact for those offsets; 0 switches the path off) and the tile's first cell, which the block carries from tile to
+// tile by addition.
 // STORE: write the velocity planes.  MOM: also reduce (sum vx, sum vy, sum vz, sum |v|^2) per cell into
 // mom[ncell][4] -- the loader fused with its first consumer: with STORE = false
 // no velocity ever reaches HBM.
 template <typename T, bool VEC, bool STORE, bool MOM>
-__global__ void __launch_bounds__(kThreads)
-sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, const __grid_constant__ PhiloxKeys K,
-                    const Coef<T>* __restrict__ W, const T* __restrict__ drift, int64_t drift_stride,
-                    T* __restrict__ vx, T* __restrict__ vy, T* __restrict__ vz, T* __restrict__ mom, int mom_mode,
-                    int mom_lanes) {
+__global__ void __launch_bounds__(kThreads, 2)
+sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, uint64_t offset,
+                    const __grid_constant__ PhiloxKeys K, const CellRec<T>* __restrict__ W, T* __restrict__ vx,
+                    T* __restrict__ vy, T* __restrict__ vz, T* __restrict__ mom, int mom_mode, int mom_lanes) {
     constexpr int G = 16 / sizeof(T);
     constexpr int64_t kTile = (int64_t)kThreads * G * kGroups;
     const bool whole_groups = ppc % (uint32_t)G == 0u;                 // every 128-bit group inside one cell
     math_tables_init<T>();
-    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+    const int64_t stride = (int64_t)gridDim.x * kTile;
+    int64_t base = (int64_t)blockIdx.x * kTile;
+    // first cell of the tile and the tile's offset inside it, advanced by (stride / ppc, stride % ppc) per tile
+    int64_t cell_first = base < n ? cell_of(base, ppc, magic) : 0;
+    uint32_t rem_first = (uint32_t)(base - cell_first * (int64_t)ppc);
+    const int64_t dcell = cell_of(stride, ppc, magic);
+    const uint32_t drem = (uint32_t)(stride - dcell * (int64_t)ppc);
+    for (; base < n; base += stride) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (VEC && whole_groups && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
-            // whole tile in range and inside one 2^32 block of counters: the straight-line tile of the
-            // uniform sampler (one Philox head; float: round-1 products by constant additions), one Coef per group
+        if (VEC && whole_groups && magic32 != 0u && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
+            // the straight-line tile of the uniform sampler (one Philox head; float: round-1 products by constant additions)
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
             const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
             T ox[kGroups][G], oy[kGroups][G], oz[kGroups][G];
+            int64_t cell[kGroups];
+            RecRegs<T> rec[kGroups];
 #pragma unroll
             for (int j = 0; j < kGroups; ++j) {
-                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
-                const int64_t cell0 = cell_of(i, ppc, magic);
-                const Coef<T> C = W[cell0];
+                cell[j] = cell_first + (int64_t)__umulhi(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, magic32);
+                load_rec(W, cell[j], rec[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < kGroups; ++j) {
                 uint32_t w0[G], w1[G], w2[G], w3[G];
                 tile_group_words<T, G, kThreads>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
-                words_to_velocities<false, false>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
-                if (drift != nullptr) {
-                    const T* d = drift + 3 * cell0 * drift_stride;
-                    const T dx = d[0], dy = d[1], dz = d[2];
-#pragma unroll
-                    for (int e = 0; e < G; ++e) {
-                        ox[j][e] += dx;
-                        oy[j][e] += dy;
-                        oz[j][e] += dz;
-                    }
-                }
+                rec_velocities(w0, w1, w2, rec[j], ox[j], oy[j], oz[j]);
                 if (MOM) {
-                    T ps[4] = {T(0), T(0), T(0), T(0)};
-#pragma unroll
-                    for (int e = 0; e < G; ++e) {
-                        ps[0] += ox[j][e];
-                        ps[1] += oy[j][e];
-                        ps[2] += oz[j][e];
-                        ps[3] = fma(ox[j][e], ox[j][e], fma(oy[j][e], oy[j][e], fma(oz[j][e], oz[j][e], ps[3])));
-                    }
-                    moments_out(ps, cell0, mom_mode, mom_lanes, mom);
+                    T ps[4];
+                    group_moments<T, G>(ox[j], oy[j], oz[j], ps);
+                    moments_out(ps, cell[j], mom_mode, mom_lanes, mom, 0xffffffffu);
                 }
             }
             if (STORE) {
@@ -392,57 +452,50 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint64_t offset, co
                     store_group(vz + i, oz[j]);
                 }
             }
-            continue;
-        }
-#pragma unroll
-        for (int j = 0; j < kGroups; ++j) {
-            const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
-            if (i < n) {
-                const int64_t cell0 = cell_of(i, ppc, magic);
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < kGroups; ++j) {
+                const int64_t i = base + (int64_t)j * (kThreads * G) + (int64_t)threadIdx.x * G;
+                const bool in_range = i < n;
+                const int64_t cell0 = in_range ? cell_of(i, ppc, magic) : 0;
                 const uint32_t rem = (uint32_t)(i - cell0 * (int64_t)ppc);
+                const bool one_cell = in_range && rem + (uint32_t)G <= ppc && i + G <= n;
+                const unsigned one_cell_mask = __ballot_sync(0xffffffffu, one_cell);
                 T ox[G], oy[G], oz[G];
-                if (rem + (uint32_t)G <= ppc && i + G <= n) {
-                    const Coef<T> C = W[cell0];
-                    group_velocities<false>(offset + (uint64_t)i, K, C, ox, oy, oz);
-                    if (drift != nullptr) {
-                        const T* d = drift + 3 * cell0 * drift_stride;
-                        const T dx = d[0], dy = d[1], dz = d[2];
-#pragma unroll
-                        for (int e = 0; e < G; ++e) {
-                            ox[e] += dx;
-                            oy[e] += dy;
-                            oz[e] += dz;
-                        }
-                    }
+                if (one_cell) {
+                    RecRegs<T> rec;
+                    load_rec(W, cell0, rec);
+                    uint32_t w0[G], w1[G], w2[G], w3[G];
+                    group_words<G>(offset + (uint64_t)i, K, w0, w1, w2, w3);
+                    rec_velocities(w0, w1, w2, rec, ox, oy, oz);
                     if (MOM) {
-                        T ps[4] = {T(0), T(0), T(0), T(0)};
-#pragma unroll
-                        for (int e = 0; e < G; ++e) {
-                            ps[0] += ox[e];
-                            ps[1] += oy[e];
-                            ps[2] += oz[e];
-                            ps[3] = fma(ox[e], ox[e], fma(oy[e], oy[e], fma(oz[e], oz[e], ps[3])));
-                        }
-                        moments_out(ps, cell0, mom_mode, mom_lanes, mom);
+                        T ps[4];
+                        group_moments<T, G>(ox, oy, oz, ps);
+                        moments_out(ps, cell0, mom_mode, mom_lanes, mom, one_cell_mask);
                     }
-                } else {
+                } else if (in_range) {
 #pragma unroll
                     for (int e = 0; e < G; ++e) {
                         int64_t cell = cell0 + (int64_t)((rem + (uint32_t)e) / ppc);
                         if (i + e >= n) cell = cell0;                 // lanes past the end: stay in bounds
-                        const Coef<T> C = W[cell];
+                        const CellRec<T> R = W[cell];
                         uint32_t w0, w1, w2;
                         particle_words(offset + (uint64_t)(i + e), K, w0, w1, w2);
-                        velocity<false>(w0, w1, w2, 0u, C, ox[e], oy[e], oz[e]);
-                        if (drift != nullptr) add_drift(drift + 3 * cell * drift_stride, ox[e], oy[e], oz[e]);
+                        rec_velocity(w0, w1, w2, R, ox[e], oy[e], oz[e]);
                         if (MOM && i + e < n) {                       // only reached in kMomAtomic mode
                             T ps[4] = {ox[e], oy[e], oz[e], fma(ox[e], ox[e], fma(oy[e], oy[e], oz[e] * oz[e]))};
-                            moments_out(ps, cell, kMomAtomic, 1, mom);
+                            moments_out(ps, cell, kMomAtomic, 1, mom, 0u);
                         }
                     }
                 }
-                if (STORE) store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
+                if (STORE && in_range) store_planes<T, VEC, G>(i, n, vx, vy, vz, ox, oy, oz);
             }
+        }
+        cell_first += dcell;
+        rem_first += drem;
+        if (rem_first >= ppc) {
+            rem_first -= ppc;
+            ++cell_first;
         }
     }
 }

@@ -113,18 +113,27 @@ __device__ __forceinline__ void direction_f32(uint32_t w1, uint32_t w2, float& m
 }
 
 // FOLD: theta is already inside C.k2 / C.th4 (uniform-parameter kernels); otherwise multiply by C.theta
-// (per-cell parameters, theta = 0, or theta outside [2^-30, 2^30]).
-template <bool FOLD, bool U64 = false>
+// (per-cell parameters, theta = 0, or theta outside [2^-30, 2^30]).  DRIFT: the cell's drift (dx, dy, dz) enters as the
+// addend of the last multiply (one rounding), in every code path alike, so that a particle's value does not
+// depend on which path produced it.
+template <bool FOLD, bool U64 = false, bool DRIFT = false>
 __device__ __forceinline__ void velocity_f32(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3,
-                                             const Coef<float>& C, float& vx, float& vy, float& vz) {
+                                             const Coef<float>& C, float& vx, float& vy, float& vz,
+                                             float dx = 0.0f, float dy = 0.0f, float dz = 0.0f) {
     float V2 = speed2_f32<U64>(w0, w3, C);             // 2V
     if (!FOLD) V2 *= C.theta;
     float muh, sth, cphi, sphi;
     direction_f32(w1, w2, muh, sth, cphi, sphi);
     const float Vs = V2 * sth;
-    vx = V2 * muh;
-    vy = Vs * cphi;
-    vz = Vs * sphi;
+    if (DRIFT) {
+        vx = fmaf(V2, muh, dx);
+        vy = fmaf(Vs, cphi, dy);
+        vz = fmaf(Vs, sphi, dz);
+    } else {
+        vx = V2 * muh;
+        vy = Vs * cphi;
+        vz = Vs * sphi;
+    }
 }
 
 }  // namespace kappagen

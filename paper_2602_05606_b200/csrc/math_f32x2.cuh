@@ -23,9 +23,19 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 #define KG_MAP2(fn, v) ([&] { float a_, b_; up2((v), a_, b_); return pk2(fn(a_), fn(b_)); }())
 
+// The chain's constants as packed pairs (x, x).  Uniform parameters: splat once per kernel from the Coef in the
+// constant bank; per-cell parameters: the pairs are what the cells kernel stages in shared memory (no move needed).
+struct Coef2 {
+    f32x2 s, ms, a, mck, bk4, k2, b2, th4, theta;
+};
+__device__ __forceinline__ Coef2 splat_coef(const Coef<float>& C) {
+    return Coef2{splat2(C.s), splat2(-C.s), splat2(C.a), splat2(-C.ck), splat2(C.bk4), splat2(C.k2), splat2(C.b2),
+                 splat2(C.th4), splat2(C.theta)};
+}
+
 // 2V for two particles (see speed2_f32).
 template <bool U64>
-__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32_t w3a, uint32_t w3b, const Coef<float>& C) {
+__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32_t w3a, uint32_t w3b, const Coef2& C) {
     // 2^32 U1 and 1 - U1 (uniform1_f32, packed); U64: the fourth word refines both where the first is small
     const f32x2 ulo = U64 ? fma2(pk2((float)w3a, (float)w3b), splat2(0x1p-32f), splat2(0x1p-33f)) : splat2(0.5f);
     const f32x2 tlo = U64 ? fma2(pk2((float)(uint32_t)(~w3a), (float)(uint32_t)(~w3b)), splat2(0x1p-64f), splat2(0x1p-65f))
@@ -41,8 +51,8 @@ __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32
     G = fma2(G, p, splat2(0x1.ebc184p-2f));
     G = fma2(G, p, splat2(0x1.71565ep-1f));
     G = fma2(G, p, splat2(0x1.715476p+0f));
-    const f32x2 m_small = mul2(mul2(p, splat2(C.s)), G);
-    const f32x2 m_large = mul2(KG_MAP2(mufu_lg2, S), splat2(-C.s));
+    const f32x2 m_small = mul2(mul2(p, C.s), G);
+    const f32x2 m_large = mul2(KG_MAP2(mufu_lg2, S), C.ms);
     float pa, pb, msa, msb, mla, mlb;
     up2(p, pa, pb); up2(m_small, msa, msb); up2(m_large, mla, mlb);
     const float ma = (pa < 0.25f) ? msa : mla, mb = (pb < 0.25f) ? msb : mlb;
@@ -56,18 +66,25 @@ __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32
     float ysa, ysb, yla, ylb;
     up2(y_small, ysa, ysb); up2(y_large, yla, ylb);
     const f32x2 Y = pk2((ma < 0.5f) ? ysa : yla, (mb < 0.5f) ? ysb : ylb);
-    const f32x2 A = fma2(Y, splat2(-C.ck), splat2(C.a));
-    const f32x2 D = KG_MAP2(mufu_sqrt, fma2(A, A, mul2(Y, splat2(C.bk4))));
+    const f32x2 A = fma2(Y, C.mck, C.a);
+    const f32x2 D = KG_MAP2(mufu_sqrt, fma2(A, A, mul2(Y, C.bk4)));
     float Aa, Ab, Da, Db;
     up2(A, Aa, Ab); up2(D, Da, Db);
     const float Ta = fabsf(Aa) + Da, Tb = fabsf(Ab) + Db;
-    const f32x2 n_pos = mul2(Y, splat2(C.k2)), n_neg = mul2(pk2(Ta, Tb), splat2(C.th4));
+    const f32x2 n_pos = mul2(Y, C.k2), n_neg = mul2(pk2(Ta, Tb), C.th4);
     float npa, npb, nna, nnb;
     up2(n_pos, npa, npb); up2(n_neg, nna, nnb);
     const bool posa = Aa >= 0.0f, posb = Ab >= 0.0f;
     const f32x2 num = pk2(posa ? npa : nna, posb ? npb : nnb);
-    const f32x2 den = pk2(posa ? Ta : C.b2, posb ? Tb : C.b2);
+    float b2a, b2b;
+    up2(C.b2, b2a, b2b);
+    const f32x2 den = pk2(posa ? Ta : b2a, posb ? Tb : b2b);
     return mul2(num, KG_MAP2(mufu_rsq, mul2(num, den)));
+}
+
+template <bool U64>
+__device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32_t w3a, uint32_t w3b, const Coef<float>& C) {
+    return speed2_f32x2<U64>(w0a, w0b, w3a, w3b, splat_coef(C));
 }
 
 __device__ __forceinline__ void quadrant_f32(uint32_t w2, float sr, float cr, float& cphi, float& sphi) {
@@ -79,12 +96,14 @@ __device__ __forceinline__ void quadrant_f32(uint32_t w2, float sr, float cr, fl
     sphi = __uint_as_float(__float_as_uint(s0) ^ (wq & 0x80000000u));
 }
 
-template <bool FOLD, bool U64 = false>
+// DRIFT: (dx, dy, dz) as pairs, added by the last multiply-add (see velocity_f32).
+template <bool FOLD, bool U64 = false, bool DRIFT = false>
 __device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
-                                                  const uint32_t (&w3)[2], const Coef<float>& C, float (&vx)[2],
-                                                  float (&vy)[2], float (&vz)[2]) {
+                                                  const uint32_t (&w3)[2], const Coef2& C, float (&vx)[2],
+                                                  float (&vy)[2], float (&vz)[2], f32x2 dx = 0ull, f32x2 dy = 0ull,
+                                                  f32x2 dz = 0ull) {
     f32x2 V2 = speed2_f32x2<U64>(w0[0], w0[1], w3[0], w3[1], C);
-    if (!FOLD) V2 = mul2(V2, splat2(C.theta));
+    if (!FOLD) V2 = mul2(V2, C.theta);
     const f32x2 muh = fma2(pk2((float)(int32_t)(w1[0] ^ 0x80000000u), (float)(int32_t)(w1[1] ^ 0x80000000u)),
                            splat2(0x1p-32f), splat2(0x1p-33f));
     const f32x2 ef = pk2((float)min(w1[0], ~w1[0]), (float)min(w1[1], ~w1[1]));
@@ -105,9 +124,21 @@ __device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const
     quadrant_f32(w2[0], sra, cra, ca, sa);
     quadrant_f32(w2[1], srb, crb, cb, sb);
     const f32x2 Vs = mul2(V2, sth);
-    up2(mul2(V2, muh), vx[0], vx[1]);
-    up2(mul2(Vs, pk2(ca, cb)), vy[0], vy[1]);
-    up2(mul2(Vs, pk2(sa, sb)), vz[0], vz[1]);
+    if (DRIFT) {
+        up2(fma2(V2, muh, dx), vx[0], vx[1]);
+        up2(fma2(Vs, pk2(ca, cb), dy), vy[0], vy[1]);
+        up2(fma2(Vs, pk2(sa, sb), dz), vz[0], vz[1]);
+    } else {
+        up2(mul2(V2, muh), vx[0], vx[1]);
+        up2(mul2(Vs, pk2(ca, cb)), vy[0], vy[1]);
+        up2(mul2(Vs, pk2(sa, sb)), vz[0], vz[1]);
+    }
+}
+template <bool FOLD, bool U64 = false>
+__device__ __forceinline__ void velocity_pair_f32(const uint32_t (&w0)[2], const uint32_t (&w1)[2], const uint32_t (&w2)[2],
+                                                  const uint32_t (&w3)[2], const Coef<float>& C, float (&vx)[2],
+                                                  float (&vy)[2], float (&vz)[2]) {
+    velocity_pair_f32<FOLD, U64, false>(w0, w1, w2, w3, splat_coef(C), vx, vy, vz);
 }
 
 }  // namespace kappagen

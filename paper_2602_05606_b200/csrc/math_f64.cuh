@@ -184,9 +184,11 @@ __device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef
     return C.theta * (nm * rsqrt3_f64(nm * dn));
 }
 
-template <bool U64 = false>
+// DRIFT: the cell's drift as the addend of the last multiply (one rounding), as in velocity_f32.
+template <bool U64 = false, bool DRIFT = false>
 __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3,
-                                             const Coef<double>& C, double& vx, double& vy, double& vz) {
+                                             const Coef<double>& C, double& vx, double& vy, double& vz,
+                                             double dx = 0.0, double dy = 0.0, double dz = 0.0) {
     const double V = speed_f64<U64>(w0, w3, C);
     const double x2 = u32_unit(w1);
     const double u2 = x2 - (1.0 - 0x1p-33);                                      // U2, exact
@@ -218,9 +220,15 @@ __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t 
     const double cphi = __hiloint2double(__double2hiint(c0) ^ (int)((wq + 0x40000000u) & 0x80000000u), __double2loint(c0));
     const double sphi = __hiloint2double(__double2hiint(s0) ^ (int)(wq & 0x80000000u), __double2loint(s0));
     const double Vs = (V + V) * sth;
-    vx = V * mu;
-    vy = Vs * cphi;
-    vz = Vs * sphi;
+    if (DRIFT) {
+        vx = fma(V, mu, dx);
+        vy = fma(Vs, cphi, dy);
+        vz = fma(Vs, sphi, dz);
+    } else {
+        vx = V * mu;
+        vy = Vs * cphi;
+        vz = Vs * sphi;
+    }
 }
 
 }  // namespace kappagen

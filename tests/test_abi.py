@@ -59,8 +59,8 @@ def test_argument_errors_are_reported_before_any_launch(L):
     assert g(4, 2, 16, 16, 16, 5, 0, 0, kg.F32, 16, 16, 16, 16, 1 << 20, None) == kg.EINVAL   # bad drift stride
     assert g(4, 2, None, 16, None, 0, 0, 0, kg.F32, 16, 16, 16, 16, 1 << 20, None) == kg.ENULL
     assert g(0, 64, None, None, None, 0, 0, 0, kg.F32, None, None, None, None, 0, None) == kg.OK
-    assert L.kappagen_cells_workspace_bytes(10, kg.F32) == 10 * 32
-    assert L.kappagen_cells_workspace_bytes(10, kg.F64) == 10 * 64
+    assert L.kappagen_cells_workspace_bytes(10, kg.F32) == 10 * 48      # one 12-value record per cell
+    assert L.kappagen_cells_workspace_bytes(10, kg.F64) == 10 * 96
     assert L.kappagen_words(-3, 0, 0, None, None, None, None) == kg.EINVAL
     assert L.kappagen_words(3, 0, 0, None, None, None, None) == kg.ENULL
 
