@@ -110,6 +110,59 @@ int kappagen_sample_cells_moments(int64_t ncell, int32_t ppc, const void* kappa,
 int kappagen_sample_host(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
                          int dtype, void* vx_host, void* vy_host, void* vz_host);
 
+/* kappagen_sample_host without any allocation or stream creation inside the call (many small batches pay
+ * neither): the caller supplies the device staging workspace and the two streams the chunks alternate on.
+ *  workspace : device, at least kappagen_sample_host_workspace_bytes(n, dtype) bytes, 256-byte aligned
+ *              (two buffers of three chunk planes; a chunk is min(n, 2^22) particles).
+ *  stream_a, stream_b : two distinct cudaStream_t (as void*); both are synchronised before the call returns,
+ *              so the host arrays are complete on return.  KAPPAGEN_EINVAL if they are equal.
+ * Values, chunking and errors as kappagen_sample_host. */
+int kappagen_sample_host_ws(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset,
+                            int dtype, void* vx_host, void* vy_host, void* vz_host,
+                            void* workspace, size_t workspace_bytes, void* stream_a, void* stream_b);
+size_t kappagen_sample_host_workspace_bytes(int64_t n, int dtype);
+
+/* The PIC particle loader (second half; "initialization stage", PAPER.md:15;
+ * 10^2-10^3 particles per cell): kappagen_sample_cells that writes, instead of three SoA planes,
+ * one array-of-structures RECORD per particle, position and velocity together, 8 elements of `dtype`
+ * (32 bytes float / 64 bytes double):
+ *     { fx, fy, fz, cell_id, vx, vy, vz, weight }
+ *  fx,fy,fz : the particle's offset inside its cell in units of the cell size, uniform in (0,1).  Positions are not
+ *             in the paper; reading R22: they come from a SECOND Philox4x32-10 block of the same particle,
+ *             counter (lo32 g, hi32 g, 0, 2), same key (the velocity block has counter word 3 = 0, the rejection
+ *             baseline 1), words 0,1,2 -> x,y,z as midpoint uniforms that the element type holds exactly:
+ *             float ((w >> 9) + 1/2)/2^23, double (w + 1/2)/2^32.  Bit-exact against the oracle.
+ *  cell_id  : cell_base + cell as a signed integer of the element's width (int32 / int64), stored in the
+ *             element's bits (reinterpret, not convert).  float: cell_base + ncell <= 2^31.
+ *  vx,vy,vz : exactly kappagen_sample_cells' values (drift included).
+ *  weight   : weight[cell] (device, [ncell] elements of `dtype`) or 1 when weight == NULL.
+ *  records  : device, [ncell*ppc][8] elements of `dtype`, 16-byte aligned.
+ * Whole tiles leave the SM as bulk asynchronous copies (cp.async.bulk) out of shared memory, 4 KB (float) per warp
+ * and instruction, so that the interleaved record is still written in full lines.
+ * kappa, theta, drift, drift_stride, seed, offset, workspace, errors: as kappagen_sample_cells. */
+int kappagen_load_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                        const void* drift, int64_t drift_stride, const void* weight, int64_t cell_base,
+                        uint64_t seed, uint64_t offset, int dtype, void* records,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
+/* Measurement hook: steps S1 and S6 alone -- the three Philox words each particle consumes, written as three uint32
+ * planes (12 bytes per particle) by the float sampler's tile walk with 128-bit stores, S2-S5 stripped.  Its rate is
+ * the ceiling of kappagen_sample(F32) on this device (bench.py reports the sampler as a fraction of it).
+ * w0,w1,w2: device, [n] uint32, 4-byte aligned (16-byte aligned planes take the vector path).  Same words as
+ * kappagen_words. */
+int kappagen_philox_planes(int64_t n, uint64_t seed, uint64_t offset,
+                           uint32_t* w0, uint32_t* w1, uint32_t* w2, void* stream);
+
+/* Measurement hook: issue-rate probe behind the "alu" rooflines of DESIGN.md section 5 and profiles/r02_pipe_rates.md.
+ * Runs a register-only loop of a fixed instruction mix (eight independent chains per kind: IMAD.WIDE.U32, LOP3, FFMA2,
+ * MUFU.EX2, DFMA, IMAD) on every SM with `warps_per_scheduler` warps per SM sub-partition and reports the mean
+ * cycles per loop iteration per warp (clock64 around the loop, averaged over blocks).
+ *  mix   : 0 .. kappagen_pipe_probe_count()-1; the instruction counts of that mix come back in counts[6]
+ *          (host, order as above; may be NULL).
+ *  iters : loop trips (>= 1).   cycles_per_iter: host pointer, required.   Synchronous; runs on the legacy stream. */
+int kappagen_pipe_probe(int mix, int warps_per_scheduler, int iters, double* cycles_per_iter, int* counts);
+int kappagen_pipe_probe_count(void);
+
 /* GPU baseline, NOT the paper's method: the "standard method" it is compared with (PAPER.md:17,
  * :180, :219-224): v = theta sqrt(kappa/(2g)) (n1,n2,n3), n_j ~ N(0,1) by Box-Muller, g ~
  * Gamma(kappa-1/2) by the Marsaglia-Tsang rejection loop.  Samples the EXACT Kappa distribution;

@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
             L.oracle_sample_cells.argtypes = [i64, i32, _f64p, _f64p, _f64p, i64, u64, u64,
                                               _f64p, _f64p, _f64p, _f64p, _f64p, _f64p]
             L.oracle_sample_cells.restype = ctypes.c_int
+            L.oracle_positions.argtypes = [i64, u64, u64, ctypes.c_int, _f64p, _f64p, _f64p]
+            L.oracle_positions.restype = ctypes.c_int
             L.oracle_cells_moments.argtypes = [i64, i32, _f64p, _f64p, _f64p, i64, u64, u64, _f64p, _f64p]
             L.oracle_cells_moments.restype = ctypes.c_int
             L.oracle_x_of_w0w3.argtypes = [i64, _u32p, _u32p, f64, _f64p]
@@ -178,6 +180,15 @@ def sample_cells(ppc: int, kappa, theta, drift, drift_stride: int, seed: int, of
     if rc != 0:
         raise ValueError("bad arguments")
     return (tuple(v), tuple(t)) if thermal else tuple(v)
+
+
+def positions(n: int, seed: int, offset: int = 0, bits: int = 23):
+    """Offsets (fx, fy, fz) in (0,1) of the particles inside their cells: the second Philox block of each particle
+    (counter word 3 = 2), midpoint uniforms of `bits` bits (23: exact in float, 32: exact in double); reading R22."""
+    f = [np.empty(n, dtype=np.float64) for _ in range(3)]
+    if lib().oracle_positions(n, seed, offset, bits, _p64(f[0]), _p64(f[1]), _p64(f[2])) != 0:
+        raise ValueError("bad arguments")
+    return tuple(f)
 
 
 def cells_moments(ppc: int, kappa, theta, drift, drift_stride: int, seed: int, offset: int = 0):

@@ -32,7 +32,9 @@
 // trip through Eq. (A11), exact CDF Eq. (3), Eq. (5), 50-digit mpmath evaluation of Table I);
 // the literal evaluator (x_literal, dir_literal, oracle_sample_literal) in tests/test_oracle_literal.py
 // (Table I lines 5-10 typed once more in 50-digit mpmath; agreement with oracle_sample in the bulk;
-// polar axis and the (cos, sin) assignment from the top bits of the words).
+// polar axis and the (cos, sin) assignment from the top bits of the words); oracle_positions in
+// tests/test_oracle_positions.py (an independent pure-Python Philox checked against the published vectors, the
+// distinctness of the position block, exact representability, uniformity and independence of the velocity stream).
 //
 // Parity status: every exported function below is pinned; none is "parity unpinned".
 
@@ -350,6 +352,25 @@ int oracle_sample_literal(int64_t n, double kappa, double theta, uint64_t seed, 
         vx[i] = (double)(V * d.mu);
         vy[i] = (double)(V * d.sth * d.cphi);
         vz[i] = (double)(V * d.sth * d.sphi);
+    }
+    return 0;
+}
+
+// Positions of the PIC particle record (kappagen_load_cells; reading R22 -- they are not in the paper):
+// the offset of particle g inside its cell, in units of the cell size, from a SECOND Philox block of the same
+// particle, counter (lo32 g, hi32 g, 0, 2), same key; words 0,1,2 -> x,y,z as midpoint uniforms of `bits` bits,
+// ((w >> (32 - bits)) + 1/2) / 2^bits: bits = 23 is what a float holds exactly, bits = 32 a double.
+int oracle_positions(int64_t n, uint64_t seed, uint64_t offset, int bits, double* fx, double* fy, double* fz) {
+    if (n < 0 || bits < 1 || bits > 32) return -1;
+    const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
+    double* f[3] = {fx, fy, fz};
+    for (int64_t i = 0; i < n; ++i) {
+        const uint64_t g = offset + (uint64_t)i;
+        const uint32_t ctr[4] = {(uint32_t)(g & 0xffffffffu), (uint32_t)(g >> 32), 0u, 2u};
+        uint32_t w[4];
+        philox4x32_10(ctr, key, w);
+        for (int q = 0; q < 3; ++q)
+            f[q][i] = (double)(((ld)(w[q] >> (32 - bits)) + 0.5L) / ldexpl(1.0L, bits));
     }
     return 0;
 }

@@ -10,6 +10,8 @@
 #include "baseline_mt.cuh"
 #include "host_params.hpp"
 #include "kernels.cuh"
+#include "load_cells.cuh"
+#include "pipe_probe.cuh"
 
 namespace kappagen {
 
@@ -540,29 +542,23 @@ extern "C" int kappagen_velocity_of_words_tile(int64_t n, const uint32_t* w0, co
 
 // End-to-end path: host destination, chunked, double-buffered (the copy of chunk c overlaps the kernel
 // of chunk c+1 on the other stream).
-extern "C" int kappagen_sample_host(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
-                                    void* vx_host, void* vy_host, void* vz_host) {
-    const char* fn = "kappagen_sample_host";
-    bool vec = false;
-    int rc = check_planes(fn, n, dtype, vx_host, vy_host, vz_host, &vec);
-    if (rc != KAPPAGEN_OK) return rc;
-    if (!domain_ok(kappa, theta)) {
-        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
-        return KAPPAGEN_EINVAL;
-    }
-    if (n == 0) return KAPPAGEN_OK;
+static constexpr int64_t kHostChunk = (int64_t)1 << 22;              // particles: 48 / 96 MiB of output per chunk
+static size_t host_plane_bytes(int64_t n, int dtype) {
+    const int64_t chunk = n < kHostChunk ? n : kHostChunk;
+    return (((size_t)chunk * elem_size(dtype)) + 255) & ~(size_t)255;
+}
+extern "C" size_t kappagen_sample_host_workspace_bytes(int64_t n, int dtype) {
+    if (n <= 0 || (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64)) return 0;
+    return 6 * host_plane_bytes(n, dtype);
+}
+
+// dev: 6 planes of host_plane_bytes; st[0], st[1]: the two streams; both synchronised on return.
+static int sample_host_on(const char* fn, int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                          void* vx_host, void* vy_host, void* vz_host, char* dev, cudaStream_t* st) {
     const size_t es = elem_size(dtype);
-    const int64_t chunk = n < ((int64_t)1 << 22) ? n : ((int64_t)1 << 22);   // 48 / 96 MiB of output per chunk
-    const size_t plane = (((size_t)chunk * es) + 255) & ~(size_t)255;
-    char* dev = nullptr;
-    cudaStream_t st[2] = {nullptr, nullptr};
-    KG_CUDA(cudaMalloc(&dev, 6 * plane));
+    const int64_t chunk = n < kHostChunk ? n : kHostChunk;
+    const size_t plane = host_plane_bytes(n, dtype);
     int status = KAPPAGEN_OK;
-    for (int b = 0; b < 2 && status == KAPPAGEN_OK; ++b)
-        if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) {
-            set_error("%s: cudaStreamCreate failed", fn);
-            status = KAPPAGEN_ECUDA;
-        }
     int64_t done = 0;
     for (int c = 0; done < n && status == KAPPAGEN_OK; ++c) {
         const int b = c & 1;
@@ -581,14 +577,233 @@ extern "C" int kappagen_sample_host(int64_t n, double kappa, double theta, uint6
         done += m;
     }
     for (int b = 0; b < 2; ++b) {
-        if (st[b]) {
-            if (cudaStreamSynchronize(st[b]) != cudaSuccess && status == KAPPAGEN_OK) {
-                set_error("%s: stream synchronize failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
-                status = KAPPAGEN_ECUDA;
-            }
-            cudaStreamDestroy(st[b]);
+        if (cudaStreamSynchronize(st[b]) != cudaSuccess && status == KAPPAGEN_OK) {
+            set_error("%s: stream synchronize failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
+            status = KAPPAGEN_ECUDA;
         }
     }
+    return status;
+}
+
+static int sample_host_checks(const char* fn, int64_t n, double kappa, double theta, int dtype, void* vx, void* vy, void* vz) {
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_sample_host(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                                    void* vx_host, void* vy_host, void* vz_host) {
+    const char* fn = "kappagen_sample_host";
+    int rc = sample_host_checks(fn, n, kappa, theta, dtype, vx_host, vy_host, vz_host);
+    if (rc != KAPPAGEN_OK || n == 0) return rc;
+    char* dev = nullptr;
+    cudaStream_t st[2] = {nullptr, nullptr};
+    KG_CUDA(cudaMalloc(&dev, kappagen_sample_host_workspace_bytes(n, dtype)));
+    int status = KAPPAGEN_OK;
+    for (int b = 0; b < 2 && status == KAPPAGEN_OK; ++b)
+        if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) {
+            set_error("%s: cudaStreamCreate failed", fn);
+            status = KAPPAGEN_ECUDA;
+        }
+    if (status == KAPPAGEN_OK) status = sample_host_on(fn, n, kappa, theta, seed, offset, dtype, vx_host, vy_host, vz_host, dev, st);
+    for (int b = 0; b < 2; ++b)
+        if (st[b]) cudaStreamDestroy(st[b]);
     cudaFree(dev);
+    return status;
+}
+
+extern "C" int kappagen_sample_host_ws(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,
+                                       void* vx_host, void* vy_host, void* vz_host, void* workspace, size_t workspace_bytes,
+                                       void* stream_a, void* stream_b) {
+    const char* fn = "kappagen_sample_host_ws";
+    int rc = sample_host_checks(fn, n, kappa, theta, dtype, vx_host, vy_host, vz_host);
+    if (rc != KAPPAGEN_OK || n == 0) return rc;
+    if (stream_a == stream_b) {
+        set_error("%s: the two streams must differ (the chunks alternate between them)", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (!workspace || workspace_bytes < kappagen_sample_host_workspace_bytes(n, dtype) || !aligned_to(workspace, 256)) {
+        set_error("%s: workspace NULL, not 256-byte aligned or smaller than %zu bytes", fn, kappagen_sample_host_workspace_bytes(n, dtype));
+        return KAPPAGEN_EWORKSPACE;
+    }
+    cudaStream_t st[2] = {(cudaStream_t)stream_a, (cudaStream_t)stream_b};
+    return sample_host_on(fn, n, kappa, theta, seed, offset, dtype, vx_host, vy_host, vz_host, (char*)workspace, st);
+}
+
+// ---- kappagen_load_cells: per-cell velocities and positions as one AoS record per particle (load_cells.cuh)
+static void cells_magics(int64_t n, int32_t ppc, int64_t tile, uint64_t* magic, uint32_t* magic32) {
+    const uint64_t up = (uint64_t)ppc;
+    *magic = ~0ull;
+    if ((up & (up - 1)) == 0) {
+        *magic = 0;
+        while ((1ull << *magic) < up) ++*magic;
+    } else if ((uint64_t)n <= (~0ull) / up) {
+        *magic = (~0ull) / up + 1;
+    }
+    *magic32 = 0;
+    if (up >= 2 && ((uint64_t)tile + up) * up < (1ull << 32)) *magic32 = (uint32_t)(((1ull << 32) + up - 1) / up);
+}
+
+template <typename T, bool HASW>
+static int launch_load_as(int64_t n, int32_t ppc, uint64_t offset, const PhiloxKeys& K, const CellRec<T>* W, const T* weight,
+                          int64_t cell_base, T* out, cudaStream_t st) {
+    constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
+    KG_CUDA(cudaFuncSetAttribute(load_cells_kernel<T, HASW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLoadSmemBytes));
+    uint64_t magic;
+    uint32_t magic32;
+    cells_magics(n, ppc, tile, &magic, &magic32);
+    PhiloxKeys Kpos = K;
+    Kpos.k1[0] ^= 2u;                                                 // counter word 3 = 2: the position block (reading R22)
+    int grid = 0, rc;
+    if ((rc = grid_for<load_cells_kernel<T, HASW>>((n + tile - 1) / tile, &grid, kThreads, kLoadSmemBytes)) != KAPPAGEN_OK) return rc;
+    load_cells_kernel<T, HASW><<<grid, kThreads, kLoadSmemBytes, st>>>(n, (uint32_t)ppc, magic, magic32, offset, K, Kpos, W, weight,
+                                                                      cell_base, out);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+template <typename T>
+static int launch_load(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift, int64_t drift_stride,
+                       const T* weight, int64_t cell_base, uint64_t offset, const PhiloxKeys& K, T* out, CellRec<T>* W,
+                       cudaStream_t st) {
+    const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
+    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, drift, drift_stride, W, nullptr);
+    KG_CUDA(cudaGetLastError());
+    const int64_t n = ncell * (int64_t)ppc;
+    return weight ? launch_load_as<T, true>(n, ppc, offset, K, W, weight, cell_base, out, st)
+                  : launch_load_as<T, false>(n, ppc, offset, K, W, weight, cell_base, out, st);
+}
+
+extern "C" int kappagen_load_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta, const void* drift,
+                                   int64_t drift_stride, const void* weight, int64_t cell_base, uint64_t seed, uint64_t offset,
+                                   int dtype, void* records, void* workspace, size_t workspace_bytes, void* stream) {
+    const char* fn = "kappagen_load_cells";
+    if (ncell < 0 || ppc < 0 || cell_base < 0) {
+        set_error("%s: negative ncell, ppc or cell_base", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (ncell > 0 && ppc > 0 && ncell > INT64_MAX / 8 / ppc) {
+        set_error("%s: ncell*ppc*8 overflows", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64) {
+        set_error("%s: dtype %d is neither KAPPAGEN_F32 nor KAPPAGEN_F64", fn, dtype);
+        return KAPPAGEN_EINVAL;
+    }
+    if (cell_base > INT64_MAX - ncell || (dtype == KAPPAGEN_F32 && cell_base + ncell > ((int64_t)1 << 31))) {
+        set_error("%s: cell_base + ncell does not fit the record's integer (int32 for float records)", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (drift != nullptr && drift_stride != 0 && drift_stride != 1) {
+        set_error("%s: drift_stride must be 0 (shared) or 1 (per cell), got %lld", fn, (long long)drift_stride);
+        return KAPPAGEN_EINVAL;
+    }
+    if (ncell == 0 || ppc == 0) return KAPPAGEN_OK;
+    if (!kappa || !theta || !records) {
+        set_error("%s: NULL kappa, theta or records", fn);
+        return KAPPAGEN_ENULL;
+    }
+    const size_t es = elem_size(dtype);
+    if (!aligned_to(kappa, es) || !aligned_to(theta, es) || (drift && !aligned_to(drift, es)) || (weight && !aligned_to(weight, es)) ||
+        !aligned_to(records, 16)) {
+        set_error("%s: kappa/theta/drift/weight not aligned to the element size, or records not 16-byte aligned", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    if (!workspace || workspace_bytes < kappagen_cells_workspace_bytes(ncell, dtype) || !aligned_to(workspace, 16)) {
+        set_error("%s: workspace NULL, misaligned or smaller than %zu bytes", fn, kappagen_cells_workspace_bytes(ncell, dtype));
+        return KAPPAGEN_EWORKSPACE;
+    }
+    const PhiloxKeys K = philox_expand_keys(seed);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32)
+        return launch_load<float>(ncell, ppc, (const float*)kappa, (const float*)theta, (const float*)drift, drift_stride,
+                                  (const float*)weight, cell_base, offset, K, (float*)records, (CellRec<float>*)workspace, st);
+    return launch_load<double>(ncell, ppc, (const double*)kappa, (const double*)theta, (const double*)drift, drift_stride,
+                               (const double*)weight, cell_base, offset, K, (double*)records, (CellRec<double>*)workspace, st);
+}
+
+// ---- measurement hooks (include/kappagen.h): the Philox + store ceiling and the pipe issue-rate probe
+extern "C" int kappagen_philox_planes(int64_t n, uint64_t seed, uint64_t offset, uint32_t* w0, uint32_t* w1, uint32_t* w2,
+                                      void* stream) {
+    const char* fn = "kappagen_philox_planes";
+    if (n < 0) {
+        set_error("%s: negative count", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!w0 || !w1 || !w2) {
+        set_error("%s: NULL output", fn);
+        return KAPPAGEN_ENULL;
+    }
+    if (!aligned_to(w0, 4) || !aligned_to(w1, 4) || !aligned_to(w2, 4)) {
+        set_error("%s: outputs must be 4-byte aligned", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    const bool vec = aligned_to(w0, 16) && aligned_to(w1, 16) && aligned_to(w2, 16);
+    constexpr int threads = TileTraits<float>::threads;
+    constexpr int64_t tile = (int64_t)threads * 4 * TileTraits<float>::groups;
+    const PhiloxKeys K = philox_expand_keys(seed);
+    cudaStream_t st = (cudaStream_t)stream;
+    int grid = 0, rc;
+    if (vec) {
+        if ((rc = grid_for<philox_planes_kernel<true>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+        philox_planes_kernel<true><<<grid, threads, 0, st>>>(n, offset, K, w0, w1, w2);
+    } else {
+        if ((rc = grid_for<philox_planes_kernel<false>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+        philox_planes_kernel<false><<<grid, threads, 0, st>>>(n, offset, K, w0, w1, w2);
+    }
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_pipe_probe_count(void) { return kPipeMixCount; }
+
+extern "C" int kappagen_pipe_probe(int mix, int warps_per_scheduler, int iters, double* cycles_per_iter, int* counts) {
+    const char* fn = "kappagen_pipe_probe";
+    if (mix < 0 || mix >= kPipeMixCount || warps_per_scheduler < 1 || warps_per_scheduler > 8 || iters < 1) {
+        set_error("%s: need 0 <= mix < %d, 1 <= warps_per_scheduler <= 8, iters >= 1", fn, kPipeMixCount);
+        return KAPPAGEN_EINVAL;
+    }
+    if (!cycles_per_iter) {
+        set_error("%s: NULL result pointer", fn);
+        return KAPPAGEN_ENULL;
+    }
+    static PipeProbeFn table[kPipeMixCount] = {};
+    if (table[0] == nullptr) PipeProbeTable<0>::fill(table);
+    if (counts) {
+        const PipeMix M = kPipeMixes[mix];
+        counts[0] = M.wide; counts[1] = M.lop3; counts[2] = M.ffma2; counts[3] = M.mufu; counts[4] = M.dfma; counts[5] = M.imad;
+    }
+    int dev = 0, sms = 0;
+    KG_CUDA(cudaGetDevice(&dev));
+    KG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int threads = warps_per_scheduler * 4 * 32;                 // one block per SM, 4 sub-partitions
+    uint32_t* sink = nullptr;
+    long long* cyc = nullptr;
+    KG_CUDA(cudaMalloc(&sink, 1024 * sizeof(uint32_t)));
+    if (cudaMalloc(&cyc, (size_t)sms * sizeof(long long)) != cudaSuccess) {
+        cudaFree(sink);
+        set_error("%s: cudaMalloc failed", fn);
+        return KAPPAGEN_ECUDA;
+    }
+    int status = KAPPAGEN_OK;
+    long long* host = new long long[sms];
+    for (int pass = 0; pass < 2; ++pass) table[mix]<<<sms, threads>>>(iters, 1u, sink, cyc);   // the second pass is timed warm
+    if (cudaMemcpy(host, cyc, (size_t)sms * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
+        set_error("%s: kernel or copy failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
+        status = KAPPAGEN_ECUDA;
+    } else {
+        double mean = 0.0;
+        for (int b = 0; b < sms; ++b) mean += (double)host[b];
+        *cycles_per_iter = mean / sms / iters / warps_per_scheduler;
+    }
+    delete[] host;
+    cudaFree(sink);
+    cudaFree(cyc);
     return status;
 }

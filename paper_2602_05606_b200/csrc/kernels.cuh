@@ -663,6 +663,57 @@ words_tile_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys
     }
 }
 
+// kappagen_philox_planes: S1 and S6 of sample_kernel<float> with S2-S5 stripped -- the same tile walk, the same
+// whole-tile test and word functions, the three words stored as three uint32 planes with 128-bit streaming stores
+// (12 bytes per particle, like the float sampler).  The measured ceiling of the float sampler.
+template <bool VEC>
+__global__ void __launch_bounds__(TileTraits<float>::threads, TileTraits<float>::minb)
+philox_planes_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxKeys K, uint32_t* __restrict__ o0,
+                     uint32_t* __restrict__ o1, uint32_t* __restrict__ o2) {
+    constexpr int G = 4;
+    constexpr int NG = TileTraits<float>::groups;
+    constexpr int kT = TileTraits<float>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        const uint64_t g_tile = offset + (uint64_t)base;
+        if (VEC && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
+            const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
+            const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
+            const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
+            uint32_t w0[NG][G], w1[NG][G], w2[NG][G];
+#pragma unroll
+            for (int j = 0; j < NG; ++j) {
+                uint32_t w3[G];
+                tile_group_words<float, G>(lo_first, q_first, j, H, K, w0[j], w1[j], w2[j], w3);
+            }
+#pragma unroll
+            for (int j = 0; j < NG; ++j) {
+                const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+                __stcs(reinterpret_cast<uint4*>(o0 + i), make_uint4(w0[j][0], w0[j][1], w0[j][2], w0[j][3]));
+                __stcs(reinterpret_cast<uint4*>(o1 + i), make_uint4(w1[j][0], w1[j][1], w1[j][2], w1[j][3]));
+                __stcs(reinterpret_cast<uint4*>(o2 + i), make_uint4(w2[j][0], w2[j][1], w2[j][2], w2[j][3]));
+            }
+            continue;
+        }
+#pragma unroll 1
+        for (int j = 0; j < NG; ++j) {
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+            if (i < n) {
+                uint32_t w0[G], w1[G], w2[G], w3[G];
+                group_words<G>(offset + (uint64_t)i, K, w0, w1, w2, w3);
+#pragma unroll
+                for (int e = 0; e < G; ++e) {
+                    if (i + e < n) {
+                        o0[i + e] = w0[e];
+                        o1[i + e] = w1[e];
+                        o2[i + e] = w2[e];
+                    }
+                }
+            }
+        }
+    }
+}
+
 // S2-S6 on caller-chosen words through the code sample_kernel<T> ships: every thread takes the NG groups of
 // a tile in one straight line through words_to_velocities (float: the packed pairs of math_f32x2.cuh; double:
 // the 2 NG interleaved chains), exactly as the whole-tile path instantiates them -- only the source of the

@@ -54,6 +54,12 @@ def lib() -> ctypes.CDLL:
         L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
         L.kappagen_cells_workspace_bytes.restype = sz
         L.kappagen_sample_host.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp]
+        L.kappagen_sample_host_ws.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp, sz, vp, vp]
+        L.kappagen_sample_host_workspace_bytes.argtypes = [i64, ci]
+        L.kappagen_sample_host_workspace_bytes.restype = sz
+        L.kappagen_load_cells.argtypes = [i64, i32, vp, vp, vp, i64, vp, i64, u64, u64, ci, vp, vp, sz, vp]
+        L.kappagen_philox_planes.argtypes = [i64, u64, u64, vp, vp, vp, vp]
+        L.kappagen_pipe_probe.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ci)]
         L.kappagen_baseline_mt.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp, vp]
         L.kappagen_words.argtypes = [i64, u64, u64, vp, vp, vp, vp]
         L.kappagen_words_tile.argtypes = [i64, u64, u64, ci, vp, vp, vp, vp, vp]
@@ -65,7 +71,8 @@ def lib() -> ctypes.CDLL:
         for name in ("kappagen_speed_histogram", "kappagen_relative_entropy", "kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
                      "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version",
-                     "kappagen_words_tile", "kappagen_velocity_of_words_tile"):
+                     "kappagen_words_tile", "kappagen_velocity_of_words_tile", "kappagen_sample_host_ws",
+                     "kappagen_load_cells", "kappagen_philox_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -233,6 +240,75 @@ def sample_host(n: int, kappa: float, theta: float, seed: int, offset: int = 0, 
             raise ValueError("sample_host needs contiguous CPU tensors of the requested dtype")
     _check(lib().kappagen_sample_host(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr()))
     return vx, vy, vz
+
+
+def sample_host_workspace_bytes(n: int, dtype="f32") -> int:
+    return int(lib().kappagen_sample_host_workspace_bytes(n, _dtype_code(dtype)))
+
+
+def sample_host_ws(n: int, kappa: float, theta: float, seed: int, offset: int, dtype, out, workspace, stream_a, stream_b):
+    """kappagen_sample_host_ws: as sample_host, with the caller's device staging workspace (uint8 CUDA tensor) and two
+    streams; nothing is allocated or created inside the call."""
+    code = _dtype_code(dtype)
+    vx, vy, vz = out
+    for t in (vx, vy, vz):
+        if t.is_cuda or t.dtype != _torch_dtype(code) or t.numel() < n or not t.is_contiguous():
+            raise ValueError("sample_host_ws needs contiguous CPU tensors of the requested dtype")
+    _dev(workspace, None, 0, "workspace")
+    _check(lib().kappagen_sample_host_ws(n, kappa, theta, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
+                                         workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                         _stream(stream_a), _stream(stream_b)))
+    return vx, vy, vz
+
+
+def load_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0, weight=None,
+               cell_base: int = 0, seed: int = 0, offset: int = 0, out=None, workspace=None, stream=None):
+    """kappagen_load_cells: one record {fx, fy, fz, cell_id, vx, vy, vz, weight} per particle; returns records[n, 8]
+    (the cell id sits in column 3 as integer BITS: view it with .view(torch.int32 / torch.int64))."""
+    code, ncell = _cell_inputs(ppc, kappa, theta, drift, drift_stride)
+    n = ncell * ppc
+    if weight is not None:
+        _dev(weight, kappa.dtype, ncell, "weight")
+    if out is None:
+        out = torch.empty((n, 8), dtype=kappa.dtype, device=kappa.device)
+    _dev(out, kappa.dtype, 8 * n, "records")
+    need = cells_workspace_bytes(ncell, code)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    _dev(workspace, None, 0, "workspace")
+    _same_device(kappa, weight, out, workspace)
+    _check(lib().kappagen_load_cells(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
+                                     drift.data_ptr() if drift is not None else None, drift_stride,
+                                     weight.data_ptr() if weight is not None else None, cell_base, seed, offset, code,
+                                     out.data_ptr(), workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                     _stream(stream)))
+    return out
+
+
+def philox_planes(n: int, seed: int, offset: int = 0, out=None, stream=None, device="cuda"):
+    """kappagen_philox_planes: S1 + S6 only (the float sampler's measured ceiling); three int32 tensors of uint32 bits."""
+    if out is None:
+        out = tuple(torch.empty(n, dtype=torch.int32, device=device) for _ in range(3))
+    for t in out:
+        _dev(t, (torch.int32, torch.uint32, torch.float32), n, "word plane")
+    _same_device(*out)
+    _check(lib().kappagen_philox_planes(n, seed, offset, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), _stream(stream)))
+    return out
+
+
+PIPE_KINDS = ("IMAD.WIDE.U32", "LOP3", "FFMA2", "MUFU.EX2", "DFMA", "IMAD")
+
+
+def pipe_probe_count() -> int:
+    return int(lib().kappagen_pipe_probe_count())
+
+
+def pipe_probe(mix: int, warps_per_scheduler: int = 8, iters: int = 2048):
+    """kappagen_pipe_probe: (cycles per loop iteration per warp, {kind: instructions per iteration})."""
+    cyc = ctypes.c_double()
+    counts = (ctypes.c_int * 6)()
+    _check(lib().kappagen_pipe_probe(mix, warps_per_scheduler, iters, ctypes.byref(cyc), counts))
+    return cyc.value, {k: int(c) for k, c in zip(PIPE_KINDS, counts) if c}
 
 
 def baseline_mt(n: int, kappa: float, theta: float, seed: int, offset: int = 0, dtype="f32", out=None,
