@@ -33,18 +33,77 @@ CPU_BASELINE_SAMPLE = 1 << 24          # particles of the cpu_baseline leg (~10-
 FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 FALLBACK_SM_MHZ = 1965.0               # B200 maximum SM clock (MEASURED_PEAKS.json sm_max_mhz when present)
 N_SM = 148
-# dram__bytes_read.sum + dram__bytes_write.sum of one sample_kernel launch at 2^28 particles, and the busy
-# fraction of the limiting pipe, from the ncu --set full captures summarised in profiles/r01d_kernels.md.
-NCU_TRAFFIC_BYTES = {"f32": 3162292696, "f64": 6383364976}
-NCU_PIPE_PCT = {"f32": ("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed", 77.4),
-                "f64": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 62.4)}
-# The sampler is bound by SM arithmetic, not by HBM.  Algorithmic work per particle on
-# the limiting pipe and that pipe's peak rate in thread-operations per clock per SM:
-#   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a
-#        quarter of the 128-lane FMA rate on sm_100 (measured 31.5 per clock per SM) -> 32 /clk/SM.
-#   f64: the double chain is 96 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.
+# ncu figures of one sample_kernel launch at 2^28 particles (dram__bytes_read.sum + dram__bytes_write.sum, busy
+# fraction of the pipes), copied from the `ncu --set full` captures summarised in profiles/r02_kernels.md.  They are
+# NOT measured by this run: the line prints them under "ncu" with their source so that nobody takes them for it.
+NCU_CAPTURE = {"from": "profiles/r02_kernels.md", "captured_at_commit": "see that file"}
+NCU_TRAFFIC_BYTES = {"f32": None, "f64": None}
+NCU_PIPE_PCT = {"f32": {}, "f64": {}}
+# Algorithmic work per particle on the arithmetic pipes (instruction counts from cuobjdump -sass,
+# rates from kappagen_pipe_probe = profiles/r02_pipe_rates.md), in thread-operations per clock per SM:
+#   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a quarter of
+#        the 128-lane FMA rate (probe: 4.1 cycles per warp instruction per scheduler) -> 32 /clk/SM.
+#   f64: the double chain is 87 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.  On sm_100 the FP64
+#        pipe and the FMA-heavy pipe (Philox's IMAD.WIDE) overlap only in part; their issue cycles per 32 particles sum
+#        to 87 x 2.03 + 18.2 x 4.14 + 9 x 2 scheduler cycles.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
-            "f64": (96, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+            "f64": (87, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+F64_SHARED_PORT_CYCLES = 87 * 2.03 + 18.2 * 4.14 + 9 * 2.0    # per 32 particles per scheduler: FP64 + IMAD.WIDE + IMAD/MOV
+TARGETS = {"f32": ("hbm", 0.80), "f64": ("alu", 0.70)}         # BASELINE.json north_star, last sentence
+
+
+def measured_peaks():
+    """(HBM GB/s, its source, SM MHz) from the driver-written MEASURED_PEAKS.json, else the profiling guide's fallback."""
+    peak, which, mhz = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", FALLBACK_SM_MHZ
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            j = json.load(f)
+        peak, which = float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+        mhz = float(j.get("sm_max_mhz", mhz))
+    except Exception:
+        pass
+    return peak, which, mhz
+
+
+def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None):
+    """The roofline object of sample_kernel<dtype> from this run's CUDA-event time per launch.
+    f32: the north_star's figure is the HBM write fraction (12 B per particle against the measured copy peak), so that
+    is `frac`; the pipe that actually binds the kernel is beside it under "pipe".  f64: `frac` is the FP64 pipe."""
+    es = 4 if dtype == "f32" else 8
+    peak, which, mhz = measured_peaks()
+    ops, per_clk, alu_unit, pipe = ALU_WORK[dtype]
+    rate = n / (kern_ms * 1e-3)
+    hbm = {"achieved": 3 * es * rate / 1e9, "peak": peak, "unit": "GB/s", "algorithmic_bytes_per_launch": 3 * es * n,
+           "peak_source": which}
+    hbm["frac"] = hbm["achieved"] / peak
+    alu_peak = N_SM * per_clk * mhz * 1e6 / 1e9
+    alu = {"achieved": ops * rate / 1e9, "peak": alu_peak, "unit": alu_unit, "pipe": pipe,
+           "algorithmic_ops_per_particle": ops,
+           "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5, profiles/r02_pipe_rates.md)" % (N_SM, per_clk, mhz)}
+    alu["frac"] = alu["achieved"] / alu_peak
+    kind, goal = TARGETS[dtype]
+    head = dict(hbm) if kind == "hbm" else dict(alu)
+    r = {"bound": kind, "achieved": head["achieved"], "peak": head["peak"], "unit": head["unit"], "frac": head["frac"],
+         "traffic": NCU_TRAFFIC_BYTES[dtype], "kernel": "sample_kernel<%s>" % dtype, "kernel_ms": kern_ms,
+         "kernel_ms_min": kern_min, "kernel_ms_max": kern_max, "frac_hbm": hbm["frac"], "frac_pipe": alu["frac"],
+         "hbm": hbm, "pipe": alu, "target": {"kind": kind, "frac": goal, "met": head["frac"] >= goal},
+         "ncu": {"source": NCU_CAPTURE, "dram_bytes_per_launch": NCU_TRAFFIC_BYTES[dtype], "pipe_busy_pct": NCU_PIPE_PCT[dtype]}}
+    if dtype == "f32":
+        r["bound_note"] = ("compute-bound: the FMA-heavy pipe (Philox's IMAD.WIDE + packed FMA) limits the kernel, not HBM; "
+                           "frac is the HBM write fraction the north_star asks for, frac_pipe the multiply pipe, "
+                           "frac_of_ceiling the same kernel with steps S2-S5 stripped (kappagen_philox_planes)")
+    else:
+        cyc = kern_ms * 1e-3 * mhz * 1e6 * N_SM * 4 * 32 / n           # scheduler cycles per 32 particles
+        r["shared_port"] = {"cycles_per_32_particles": cyc, "fp64_plus_fmaheavy_cycles": F64_SHARED_PORT_CYCLES,
+                            "frac": F64_SHARED_PORT_CYCLES / cyc,
+                            "note": "model: FP64 and FMA-heavy (IMAD.WIDE, IMAD) instructions overlap only in part on sm_100 "
+                                    "(profiles/r02_pipe_rates.md, mixes 11-15; ncu: fp64 + fmaheavy busy fractions add up to ~95 %); "
+                                    "this is the sum of their issue cycles per 32 particles over the elapsed cycles"}
+    if ceiling_ms is not None:
+        r["ceiling"] = {"kernel": "philox_planes_kernel (S1 + S6 only, 12 B/particle)", "kernel_ms": ceiling_ms,
+                        "particles_per_s": n / (ceiling_ms * 1e-3)}
+        r["frac_of_ceiling"] = ceiling_ms / kern_ms
+    return r
 
 
 def parse_args():
@@ -56,6 +115,8 @@ def parse_args():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / baseline / cells extra timings")
+    ap.add_argument("--pipe-rates", action="store_true",
+                    help="print the kappagen_pipe_probe table (markdown) that profiles/r02_pipe_rates.md holds, and exit")
     ap.add_argument("--sweep", action="store_true",
                     help="also time kappagen_sample over 1e6 ... 2^30 particles and kappa 1.6 ... 10 (extras.sweep)")
     return ap.parse_args()
@@ -158,13 +219,17 @@ class ClockSampler(threading.Thread):
                 pass
             time.sleep(0.005)
 
+    def mark(self):
+        self.first_timed = len(self.samples)
+
     def stop(self):
         self._stop_evt.set()
         if self.is_alive():
             self.join()
-        s = sorted(self.samples)
+        timed = sorted(self.samples[getattr(self, "first_timed", 0):])
+        s = timed if timed else sorted(self.samples)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(s)}
+                "reasons": sorted(self.reasons), "samples": len(timed), "samples_incl_warmup": len(self.samples)}
 
 
 # --------------------------------------------------------------------------- our arm
@@ -220,11 +285,12 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    sampler.start()                                     # polls every 5 ms from the warm-up on; the device stays loaded
     for s in range(max(args.warmup, 3)):
         step(s)
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler.mark()                                      # samples from here on belong to the timed region
     total_ms, per_launch = time_launches(step, args.steps, 0, torch)
     barrier()
     clocks = sampler.stop()
@@ -237,13 +303,15 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with HOST buffers (device->host copies inside the timed region)
     host = tuple(torch.empty(n, dtype=tdt, pin_memory=True) for _ in range(3))
-    kg.sample_host(n, KAPPA, THETA, SEED, rank * n, dtype, out=host)            # warm-up (also faults the pages in)
+    ws = torch.empty(kg.sample_host_workspace_bytes(n, dtype), dtype=torch.uint8, device="cuda")
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()   # the caller's: the call allocates and creates nothing
+    kg.sample_host_ws(n, KAPPA, THETA, SEED, rank * n, dtype, host, ws, sa, sb)  # warm-up (also faults the pages in)
     barrier()
     t0 = time.perf_counter()
     e2e_each = []
     for s in range(args.e2e_steps):
         t1 = time.perf_counter()
-        kg.sample_host(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, out=host)   # synchronous
+        kg.sample_host_ws(n, KAPPA, THETA, SEED, (s * world + rank) * n, dtype, host, ws, sa, sb)   # synchronous
         e2e_each.append(time.perf_counter() - t1)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
@@ -252,44 +320,34 @@ def run_ours(args):
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
     e2e_value = world * n * args.e2e_steps / float(te.item())
     checksum = float(host[0][:1024].double().abs().sum())                         # the host result is read
-    del host
+    del host, ws
 
     line = None
     if rank == 0:
-        peak, which = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-                peak, which = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
-        except Exception:
-            pass
-        hbm_achieved = 3 * es * n / (kern_ms * 1e-3) / 1e9
-        sm_mhz = FALLBACK_SM_MHZ
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-                sm_mhz = float(json.load(f)["sm_max_mhz"])
-        except Exception:
-            pass
-        ops, per_clk, alu_unit, pipe = ALU_WORK[dtype]
-        alu_achieved = ops * n / (kern_ms * 1e-3) / 1e9
-        alu_peak = N_SM * per_clk * sm_mhz * 1e6 / 1e9
+        ceiling_ms = None
+        if dtype == "f32":                               # the same launch shape with S2-S5 stripped: Philox + stores
+            wp = tuple(p.view(torch.int32) for p in planes)
+            _, cms = time_launches(lambda s: kg.philox_planes(n, SEED, s * n, out=wp, stream=stream), 10, 3, torch)
+            ceiling_ms = sum(cms) / len(cms)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": dtype, "data": "synthetic", "config": config_dict(dtype, world),
             "clocks": clocks, "gpu_launches": args.steps,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 3 * es * n * world,
-                    "steps": args.e2e_steps, "api": "kappagen_sample_host (pinned host planes)", "checksum": checksum,
-                    "ms_per_step": [round(1e3 * t, 3) for t in e2e_each],
+                    "steps": args.e2e_steps, "api": "kappagen_sample_host_ws (pinned host planes, caller's staging workspace and streams)",
+                    "checksum": checksum, "ms_per_step": [round(1e3 * t, 3) for t in e2e_each],
                     "value_at_median_step": world * n / sorted(e2e_each)[len(e2e_each) // 2]},
-            "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": alu_unit,
-                         "frac": alu_achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES[dtype], "pipe": pipe,
-                         "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5)" % (N_SM, per_clk, sm_mhz),
-                         "algorithmic_ops_per_particle": ops, "kernel": "sample_kernel<%s>" % dtype,
-                         "kernel_ms": kern_ms, "kernel_ms_min": min(per_launch), "kernel_ms_max": max(per_launch),
-                         "ncu_pipe_busy_pct": {NCU_PIPE_PCT[dtype][0]: NCU_PIPE_PCT[dtype][1]},
-                         "hbm": {"achieved": hbm_achieved, "peak": peak, "unit": "GB/s", "frac": hbm_achieved / peak,
-                                 "algorithmic_bytes_per_launch": 3 * es * n, "peak_source": which}},
+            "roofline": roofline_of(dtype, n, kern_ms, min(per_launch), max(per_launch), ceiling_ms),
         }
+        if world == 1:                                   # the other dtype of the metric ("fp32/fp64"), same workload, this run
+            other = "f64" if dtype == "f32" else "f32"
+            op = tuple(torch.empty(n, dtype=torch.float64 if other == "f64" else torch.float32, device="cuda") for _ in range(3))
+            _, oms = time_launches(lambda s: kg.sample(n, KAPPA, THETA, SEED, s * n, other, out=op, stream=stream), 20, 3, torch)
+            k = sum(oms) / len(oms)
+            line["roofline_" + other] = roofline_of(other, n, k, min(oms), max(oms))
+            line["value_" + other] = n / (k * 1e-3)
+            del op
         if world == 1 and not args.no_extras:
             line["extras"] = extras(kg, torch, dtype)
         if world == 1 and args.sweep:
@@ -347,6 +405,24 @@ def extras(kg, torch, dtype):
                                                             stream=st, store=False), 5, 2, torch)
     k = sum(ms) / len(ms)
     out["cells_moments_only_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k}
+    # the particle loader (second half): 32-byte AoS records {fx,fy,fz,cell,vx,vy,vz,w}, one kernel,
+    # against the SoA sampler followed by three strided copies into the record array (which still lacks the positions)
+    rec = torch.empty((nc, 8), dtype=torch.float32, device="cuda")
+    _, ms = time_launches(lambda s: kg.load_cells(cfg.ppc, kd, td, dd, 0, None, 0, cfg.seed, s * nc, out=rec, workspace=ws, stream=st),
+                          5, 2, torch)
+    k = sum(ms) / len(ms)
+    out["load_cells_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k, "write_GBps": 32 * nc / (k * 1e-3) / 1e9,
+                                     "record_bytes": 32}
+
+    def soa_then_interleave(s):
+        kg.sample_cells(cfg.ppc, kd, td, dd, 0, cfg.seed, s * nc, out=p32, workspace=ws, stream=st)
+        for q in range(3):
+            rec[:, 4 + q].copy_(p32[q][:nc])
+    _, ms = time_launches(soa_then_interleave, 5, 2, torch)
+    k = sum(ms) / len(ms)
+    out["sample_cells_then_interleave_f32_config4"] = {"particles_per_s": nc / (k * 1e-3), "ms": k,
+                                                       "note": "velocities only: positions, ids and weights not written"}
+    del rec
     # paper test 2 on the device: generate and bin 2^28 speeds, no velocity written
     hist = torch.zeros(512, dtype=torch.int64, device="cuda")
     for dt in ("f32", "f64"):
@@ -374,8 +450,37 @@ def sweep(kg, torch):
     return out
 
 
+def pipe_rates():
+    """The issue-rate probe of every mix at 1, 2, 4, 8 warps per scheduler: cycles per loop iteration per warp."""
+    import torch
+    from paper_2602_05606_b200 import kappagen as kg
+    if not torch.cuda.is_available():
+        raise SystemExit("--pipe-rates needs a CUDA device")
+    print("| mix | instructions per iteration | w=1 | w=2 | w=4 | w=8 | sum of single-kind costs at w=8 |")
+    print("|---|---|---|---|---|---|---|")
+    single = {}
+    rows = []
+    for mix in range(kg.pipe_probe_count()):
+        cyc = [kg.pipe_probe(mix, w, 2048) for w in (1, 2, 4, 8)]
+        counts = cyc[0][1]
+        if len(counts) == 1:
+            (kind, cnt), = counts.items()
+            single[kind] = cyc[3][0] / cnt
+        rows.append((mix, counts, [c[0] for c in cyc]))
+    for mix, counts, c in rows:
+        add = sum(single.get(k, float("nan")) * v for k, v in counts.items())
+        print("| %d | %s | %.1f | %.1f | %.1f | %.1f | %.1f |" % (mix, " + ".join("%d %s" % (v, k) for k, v in counts.items()),
+                                                               c[0], c[1], c[2], c[3], add))
+    print()
+    print("cycles per warp instruction per scheduler at w=8 (loop overhead of ~3 instructions per iteration included): " +
+          ", ".join("%s %.2f" % (k, v) for k, v in single.items()))
+
+
 def main():
     args = parse_args()
+    if args.pipe_rates:
+        pipe_rates()
+        return
     if args.impl == "reference":
         run_reference(args)
     else:
