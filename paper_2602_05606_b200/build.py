@@ -20,7 +20,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 
 def _newest_source_mtime() -> float:
-    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    # compiled sources and their headers only (fit_polynomials.py prints constants, it is not compiled)
+    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".cpp", ".hpp"))]
     paths += [os.path.join(HERE, "..", "include", "kappagen.h"), os.path.abspath(__file__)]
     return max(os.path.getmtime(p) for p in paths)
 
