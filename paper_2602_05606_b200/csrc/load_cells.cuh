@@ -9,7 +9,7 @@
 // Stores.  A thread's G particles are 128 contiguous bytes, a warp's 4 KB; written lane by lane with 128-bit stores
 // every instruction would touch 32 lines and fill a quarter of each.  Whole tiles instead assemble the warp's 4 KB in
 // shared memory and hand it to the bulk-copy engine (cp.async.bulk shared -> global, one instruction per warp and
-// group), two buffers per warp so that the copy of one group overlaps the arithmetic of the next.
+// group; one fence and one commit per tile), which drains it while the warp computes its next tile.
 #pragma once
 #include "kernels.cuh"
 
@@ -17,7 +17,7 @@ namespace kappagen {
 
 constexpr int kRecElems = 8;                                          // elements of T per particle record
 constexpr int kRecWarpBytes = 32 * 16 * 8;                            // 32 lanes x 128 bytes: one warp, one group
-constexpr int kLoadSmemBytes = (kThreads / 32) * 2 * kRecWarpBytes;   // two buffers per warp: 64 KB per block
+constexpr int kLoadSmemBytes = (kThreads / 32) * kGroups * kRecWarpBytes;   // a tile of every warp: 64 KB per block
 
 __device__ __forceinline__ float pos_offset(uint32_t w, float) {      // ((w >> 9) + 1/2) / 2^23, exact in float
     return fmaf((float)(w >> 9), 0x1p-23f, 0x1p-24f);
@@ -42,19 +42,21 @@ __device__ __forceinline__ void record_pieces(double fx, double fy, double fz, d
     pc[3] = make_double2(vz, w);
 }
 
-__device__ __forceinline__ void bulk_store_warp(void* gdst, const void* ssrc, uint32_t bytes) {
-    // generic-proxy writes to shared memory made visible to the async proxy, then one bulk copy for the warp
+// Two copies (the warp's two groups, kRecWarpBytes each, adjacent in shared memory) behind one fence, one commit.
+__device__ __forceinline__ void bulk_store_warp2(void* g0, void* g1, const void* ssrc, uint32_t bytes) {
+    // generic-proxy writes to shared memory made visible to the async proxy, then the bulk copies of the warp
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncwarp();
     if ((threadIdx.x & 31u) == 0u) {
         const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
-        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g0), "r"(s), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g1), "r"(s + bytes), "r"(bytes) : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     }
 }
-// The buffer written two groups ago may be overwritten once its copy has READ it: at most one younger copy pending.
+// The warp's buffer may be overwritten once the copies issued from it have READ it.
 __device__ __forceinline__ void bulk_wait_reuse() {
-    if ((threadIdx.x & 31u) == 0u) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    if ((threadIdx.x & 31u) == 0u) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     __syncwarp();
 }
 __device__ __forceinline__ void bulk_wait_all() {
@@ -80,34 +82,43 @@ load_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, uin
     const bool whole_groups = ppc % (uint32_t)G == 0u;
     math_tables_init<T>();
     const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
-    P* my_stage = reinterpret_cast<P*>(stage_raw + (size_t)warp * 2 * kRecWarpBytes);   // [2][32 lanes][8 pieces]
+    P* my_stage = reinterpret_cast<P*>(stage_raw + (size_t)warp * kGroups * kRecWarpBytes);   // [group][32 lanes][8 pieces]
     const int64_t stride = (int64_t)gridDim.x * kTile;
     int64_t base = (int64_t)blockIdx.x * kTile;
     int64_t cell_first = base < n ? cell_of(base, ppc, magic) : 0;
     uint32_t rem_first = (uint32_t)(base - cell_first * (int64_t)ppc);
     const int64_t dcell = cell_of(stride, ppc, magic);
     const uint32_t drem = (uint32_t)(stride - dcell * (int64_t)ppc);
-    int buf = 0;
     for (; base < n; base += stride) {
         const uint64_t g_tile = offset + (uint64_t)base;
         if (whole_groups && magic32 != 0u && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
             const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
+            // the records of both groups first: their loads fly during the first group's Philox rounds (the bulk-copy
+            // fences below are barriers for the compiler, it would not hoist them itself)
+            int64_t cells[kGroups];
+            RecRegs<T> recs[kGroups];
+            T wgts[kGroups];
 #pragma unroll
             for (int j = 0; j < kGroups; ++j) {
-                const int64_t cell = cell_first + (int64_t)__umulhi(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, magic32);
-                RecRegs<T> rec;
-                load_rec(W, cell, rec);
-                const T wgt = HASW ? __ldg(weight + cell) : T(1);
+                cells[j] = cell_first + (int64_t)__umulhi(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, magic32);
+                load_rec(W, cells[j], recs[j]);
+                wgts[j] = HASW ? __ldg(weight + cells[j]) : T(1);
+            }
+#pragma unroll
+            for (int j = 0; j < kGroups; ++j) {
+                const int64_t cell = cells[j];
+                const RecRegs<T>& rec = recs[j];
+                const T wgt = wgts[j];
                 uint32_t w0[G], w1[G], w2[G], w3[G], p0[G], p1[G], p2[G], p3[G];
                 tile_group_words<T, G, kThreads>(lo_first, q_first, j, H, K, w0, w1, w2, w3);
                 tile_group_words<T, G, kThreads>(lo_first, q_first, j, H, Kpos, p0, p1, p2, p3);
                 T ox[G], oy[G], oz[G];
                 rec_velocities(w0, w1, w2, rec, ox, oy, oz);
                 const T id = id_bits(cell_base + cell, T(0));
-                bulk_wait_reuse();                                    // the copy issued from this buffer two groups ago has read it
-                P* dst = my_stage + (size_t)buf * (kRecWarpBytes / sizeof(P)) + lane * 8u;
+                if (j == 0) bulk_wait_reuse();                        // the previous tile's copies have read the buffer
+                P* dst = my_stage + (size_t)j * (kRecWarpBytes / sizeof(P)) + lane * 8u;
 #pragma unroll
                 for (int e = 0; e < G; ++e) {
                     P pc[PP];
@@ -116,10 +127,11 @@ load_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, uin
 #pragma unroll
                     for (int u = 0; u < PP; ++u) dst[e * PP + u] = pc[u];
                 }
-                const int64_t i_warp = base + (int64_t)j * (kThreads * G) + (int64_t)(warp * 32u) * G;
-                bulk_store_warp(out + i_warp * kRecElems, my_stage + (size_t)buf * (kRecWarpBytes / sizeof(P)), (uint32_t)kRecWarpBytes);
-                buf ^= 1;
             }
+            // one fence and one commit per tile: both groups' 4 KB leave together
+            const int64_t i_warp = base + (int64_t)(warp * 32u) * G;
+            bulk_store_warp2(out + i_warp * kRecElems, out + (i_warp + (int64_t)kThreads * G) * kRecElems, my_stage,
+                             (uint32_t)kRecWarpBytes);
         } else {
             // ragged tail, tile across a 2^32 counter boundary, ppc not a multiple of G: particle by particle, the
             // scalar chain (bit-identical to the packed one), plain 128-bit stores
