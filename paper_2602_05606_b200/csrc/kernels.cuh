@@ -18,14 +18,13 @@ namespace kappagen {
 
 constexpr int kThreads = 256;
 constexpr int kGroups = 2;  // 128-bit groups per thread per tile
-// Tile shape of the sample kernels, measured on B200 (DESIGN.md "Kernels"; the macros are sweep knobs).
+// Tile shape of the sample kernels, measured on B200 (DESIGN.md section 5; the macros are sweep knobs).
 // double: 4 groups (8 particles) per thread generated in one straight line -- whole tiles inside one 2^32
-// block of counters only, one Philox head per tile, no branch between the groups, stores last -- with the
-// register budget of one 256-thread block per SM (162 registers): the chains are long and latency-bound
-// and share 64-bit constants, which the compiler keeps resident.  1.19e11 particles/s, against 9.1e10 for
-// 2 separately guarded groups at 80 registers; more warps per SM (128-thread blocks x 3, 384 x 1, 86
-// registers x 2) are all slower.  float: the same straight-line tile with 2 groups (8 particles, 96
-// registers): 2.31e11 particles/s; 1, 3 or 4 groups and min-blocks 2-4 are within 3 % below it.
+// block of counters only, one Philox head per tile, no branch between the groups, stores last -- 384 threads,
+// one block per SM (156 registers): the chains are long and share 64-bit constants, which the compiler keeps
+// resident.  1.29e11 particles/s; 64-1024 threads x 1-6 groups all lie between 2.08 and 2.43 ms per 2^28, this
+// shape is the minimum.  float: the same straight-line tile with 2 groups (8 particles, 98 registers, 2 blocks
+// per SM): 2.32e11 particles/s; 1, 3 or 4 groups and min-blocks 2-4 are within 3 % below it.
 #ifndef KG_JOINT_F64
 #define KG_JOINT_F64 1
 #endif
