@@ -74,9 +74,10 @@ int kappagen_sample_flags(int64_t n, double kappa, double theta, uint64_t seed, 
  *                 non-finite value gets NaN in all its particles (it cannot be reported synchronously).
  *  drift        : device, elements of `dtype`, or NULL (no drift).  drift_stride == 0: one shared
  *                 (dx,dy,dz) at drift[0..2]; drift_stride == 1: per cell at drift[3*cell + 0..2].
- *  workspace    : device scratch of at least kappagen_cells_workspace_bytes(ncell, dtype) bytes,
- *                 16-byte aligned; holds the per-cell Table I lines 1-4 (computed on the device in
- *                 double by a small pre-kernel on the same stream).  Contents are unspecified after.
+ *  workspace    : device scratch of at least kappagen_cells_workspace_bytes(ncell, dtype) bytes
+ *                 (48 bytes per cell for float, 96 for double), 16-byte aligned; holds one record per cell:
+ *                 the per-cell Table I lines 1-4 (computed on the device in double by a small pre-kernel
+ *                 on the same stream) and the cell's drift.  Contents are unspecified after.
  *  vx, vy, vz   : device, [ncell*ppc] elements of `dtype`. */
 int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
                           const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
