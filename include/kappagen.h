@@ -85,6 +85,17 @@ int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const v
                           void* workspace, size_t workspace_bytes, void* stream);
 size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype);
 
+/* The two halves of kappagen_sample_cells as calls of their own: "The first four lines [of Table I] are required
+ * only once".  kappagen_cells_prepare fills the workspace with the per-cell records (Table I
+ * lines 1-4 and the drift); kappagen_sample_cells_prepared draws velocities from a workspace so prepared -- as often
+ * as wanted, with any seed, offset and ppc, for the SAME ncell and dtype -- and writes exactly what
+ * kappagen_sample_cells writes.  The workspace contents are then the caller's to keep: nothing else writes them. */
+int kappagen_cells_prepare(int64_t ncell, const void* kappa, const void* theta, const void* drift,
+                           int64_t drift_stride, int dtype, void* workspace, size_t workspace_bytes, void* stream);
+int kappagen_sample_cells_prepared(int64_t ncell, int32_t ppc, uint64_t seed, uint64_t offset, int dtype,
+                                   void* vx, void* vy, void* vz,
+                                   const void* workspace, size_t workspace_bytes, void* stream);
+
 /* The loader fused with its first consumer (the step after the path in a PIC code: "initialization stage",
  * PAPER.md:15; 10^2-10^3 particles per cell): kappagen_sample_cells that ALSO reduces, per
  * cell and inside the generating kernel, the velocity moments of the cell's ppc particles (drift included)

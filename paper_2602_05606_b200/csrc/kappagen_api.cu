@@ -149,7 +149,7 @@ static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint32_t magi
 template <typename T>
 static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift,
                         int64_t drift_stride, uint64_t offset, const PhiloxKeys& K, bool vec, bool store, T* vx, T* vy,
-                        T* vz, T* mom, CellRec<T>* W, cudaStream_t st) {
+                        T* vz, T* mom, CellRec<T>* W, cudaStream_t st, bool prepare = true, bool sample = true) {
     constexpr int G = 16 / sizeof(T);
     constexpr int64_t tile = (int64_t)kThreads * G * kGroups;
     int mode = kMomNone, lanes = 1;
@@ -159,10 +159,13 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
         else if (ppc % (32 * G) == 0) { mode = kMomWarp; lanes = 32; }
         else mode = kMomAtomic;
     }
-    const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
-    cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, drift, drift_stride, W,
-                                                              (mode == kMomWarp || mode == kMomAtomic) ? mom : nullptr);
-    KG_CUDA(cudaGetLastError());
+    if (prepare) {
+        const int64_t cgrid = (ncell + kThreads - 1) / kThreads;
+        cell_coef_kernel<T><<<(unsigned)cgrid, kThreads, 0, st>>>(ncell, kappa, theta, drift, drift_stride, W,
+                                                                  (mode == kMomWarp || mode == kMomAtomic) ? mom : nullptr);
+        KG_CUDA(cudaGetLastError());
+    }
+    if (!sample) return KAPPAGEN_OK;
     const int64_t n = ncell * (int64_t)ppc;
     // cell_of(): a shift when ppc is a power of two; else floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1), exact for
     // every i with i * ppc < 2^64 (i < n); else (~0) the plain 64-bit division
@@ -633,6 +636,65 @@ extern "C" int kappagen_sample_host_ws(int64_t n, double kappa, double theta, ui
     }
     cudaStream_t st[2] = {(cudaStream_t)stream_a, (cudaStream_t)stream_b};
     return sample_host_on(fn, n, kappa, theta, seed, offset, dtype, vx_host, vy_host, vz_host, (char*)workspace, st);
+}
+
+// ---- Table I lines 1-4 "are required only once": the two halves of kappagen_sample_cells as calls of their own
+extern "C" int kappagen_cells_prepare(int64_t ncell, const void* kappa, const void* theta, const void* drift,
+                                      int64_t drift_stride, int dtype, void* workspace, size_t workspace_bytes, void* stream) {
+    const char* fn = "kappagen_cells_prepare";
+    if (ncell < 0 || (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64)) {
+        set_error("%s: negative ncell or bad dtype", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    if (drift != nullptr && drift_stride != 0 && drift_stride != 1) {
+        set_error("%s: drift_stride must be 0 (shared) or 1 (per cell), got %lld", fn, (long long)drift_stride);
+        return KAPPAGEN_EINVAL;
+    }
+    if (ncell == 0) return KAPPAGEN_OK;
+    if (!kappa || !theta) {
+        set_error("%s: NULL kappa or theta array", fn);
+        return KAPPAGEN_ENULL;
+    }
+    const size_t es = elem_size(dtype);
+    if (!aligned_to(kappa, es) || !aligned_to(theta, es) || (drift && !aligned_to(drift, es))) {
+        set_error("%s: kappa/theta/drift not aligned to the element size", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    if (!workspace || workspace_bytes < kappagen_cells_workspace_bytes(ncell, dtype) || !aligned_to(workspace, 16)) {
+        set_error("%s: workspace NULL, misaligned or smaller than %zu bytes", fn, kappagen_cells_workspace_bytes(ncell, dtype));
+        return KAPPAGEN_EWORKSPACE;
+    }
+    const PhiloxKeys K = philox_expand_keys(0);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32)
+        return launch_cells<float>(ncell, 1, (const float*)kappa, (const float*)theta, (const float*)drift, drift_stride, 0, K, false,
+                                   true, nullptr, nullptr, nullptr, nullptr, (CellRec<float>*)workspace, st, true, false);
+    return launch_cells<double>(ncell, 1, (const double*)kappa, (const double*)theta, (const double*)drift, drift_stride, 0, K, false,
+                                true, nullptr, nullptr, nullptr, nullptr, (CellRec<double>*)workspace, st, true, false);
+}
+
+extern "C" int kappagen_sample_cells_prepared(int64_t ncell, int32_t ppc, uint64_t seed, uint64_t offset, int dtype, void* vx,
+                                              void* vy, void* vz, const void* workspace, size_t workspace_bytes, void* stream) {
+    const char* fn = "kappagen_sample_cells_prepared";
+    if (ncell < 0 || ppc < 0 || (ncell > 0 && ppc > 0 && ncell > INT64_MAX / ppc)) {
+        set_error("%s: negative ncell or ppc, or ncell*ppc overflows", fn);
+        return KAPPAGEN_EINVAL;
+    }
+    bool vec = false;
+    const int64_t n = ncell * (int64_t)ppc;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK || n == 0) return rc;
+    if (!workspace || workspace_bytes < kappagen_cells_workspace_bytes(ncell, dtype) || !aligned_to(workspace, 16)) {
+        set_error("%s: workspace NULL, misaligned or smaller than %zu bytes", fn, kappagen_cells_workspace_bytes(ncell, dtype));
+        return KAPPAGEN_EWORKSPACE;
+    }
+    const PhiloxKeys K = philox_expand_keys(seed);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F32)
+        return launch_cells<float>(ncell, ppc, nullptr, nullptr, nullptr, 0, offset, K, vec, true, (float*)vx, (float*)vy, (float*)vz,
+                                   nullptr, (CellRec<float>*)const_cast<void*>(workspace), st, false, true);
+    return launch_cells<double>(ncell, ppc, nullptr, nullptr, nullptr, 0, offset, K, vec, true, (double*)vx, (double*)vy, (double*)vz,
+                                nullptr, (CellRec<double>*)const_cast<void*>(workspace), st, false, true);
 }
 
 // ---- kappagen_load_cells: per-cell velocities and positions as one AoS record per particle (load_cells.cuh)

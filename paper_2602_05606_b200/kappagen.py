@@ -51,6 +51,8 @@ def lib() -> ctypes.CDLL:
         L.kappagen_relative_entropy.argtypes = [vp, i32, f64, f64, f64, ci, ctypes.POINTER(ctypes.c_double)]
         L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
         L.kappagen_sample_cells_moments.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, vp, sz, vp]
+        L.kappagen_cells_prepare.argtypes = [i64, vp, vp, vp, i64, ci, vp, sz, vp]
+        L.kappagen_sample_cells_prepared.argtypes = [i64, i32, u64, u64, ci, vp, vp, vp, vp, sz, vp]
         L.kappagen_cells_workspace_bytes.argtypes = [i64, ci]
         L.kappagen_cells_workspace_bytes.restype = sz
         L.kappagen_sample_host.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp]
@@ -72,7 +74,7 @@ def lib() -> ctypes.CDLL:
                      "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version",
                      "kappagen_words_tile", "kappagen_velocity_of_words_tile", "kappagen_sample_host_ws",
-                     "kappagen_load_cells", "kappagen_philox_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
+                     "kappagen_load_cells", "kappagen_cells_prepare", "kappagen_sample_cells_prepared", "kappagen_philox_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -201,6 +203,32 @@ def sample_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None,
                                        drift.data_ptr() if drift is not None else None, drift_stride, seed, offset,
                                        code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), workspace.data_ptr(),
                                        workspace.numel() * workspace.element_size(), _stream(stream)))
+    return vx, vy, vz
+
+
+def cells_prepare(kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0, workspace=None, stream=None):
+    """kappagen_cells_prepare: Table I lines 1-4 per cell (+ drift) into the workspace, once; returns the workspace."""
+    code, ncell = _cell_inputs(1, kappa, theta, drift, drift_stride)
+    need = cells_workspace_bytes(ncell, code)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=kappa.device)
+    _dev(workspace, None, 0, "workspace")
+    _same_device(kappa, workspace)
+    _check(lib().kappagen_cells_prepare(ncell, kappa.data_ptr(), theta.data_ptr(), drift.data_ptr() if drift is not None else None,
+                                        drift_stride, code, workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                        _stream(stream)))
+    return workspace
+
+
+def sample_cells_prepared(ncell: int, ppc: int, workspace: torch.Tensor, seed: int = 0, offset: int = 0, dtype="f32", out=None,
+                          stream=None):
+    """kappagen_sample_cells_prepared: velocities from a workspace filled by cells_prepare."""
+    code = _dtype_code(dtype)
+    _dev(workspace, None, 0, "workspace")
+    vx, vy, vz = _planes(ncell * ppc, code, out, workspace.device)
+    _same_device(workspace, vx)
+    _check(lib().kappagen_sample_cells_prepared(ncell, ppc, seed, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(),
+                                                workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream(stream)))
     return vx, vy, vz
 
 

@@ -62,3 +62,24 @@ def test_pipe_probe_rates():
     assert 7.5 <= rates["MUFU.EX2"] <= 8.6 and 1.8 <= rates["IMAD"] <= 2.5, rates
     with pytest.raises(kg.KappagenError):
         kg.pipe_probe(kg.pipe_probe_count(), 8, 10)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_prepared_workspace_gives_the_bits_of_sample_cells(dtype):
+    """Table I lines 1-4 "are required only once": kappagen_cells_prepare once, then
+    kappagen_sample_cells_prepared for several (ppc, seed, offset) -- each bit-identical to kappagen_sample_cells."""
+    npd = np.float32 if dtype == "f32" else np.float64
+    rng = np.random.Generator(np.random.PCG64(8))
+    ncell = 777
+    kap = torch.from_numpy((1.6 + 6 * rng.random(ncell)).astype(npd)).cuda()
+    th = torch.from_numpy((0.1 + rng.random(ncell)).astype(npd)).cuda()
+    drift = torch.from_numpy((0.05 * rng.standard_normal(3 * ncell)).astype(npd)).cuda()
+    ws = kg.cells_prepare(kap, th, drift, 1)
+    for ppc, seed, offset in ((64, 1, 0), (37, 2, 2**32 - 1000), (256, 3, 12345)):
+        got = kg.sample_cells_prepared(ncell, ppc, ws, seed, offset, dtype)
+        want = kg.sample_cells(ppc, kap, th, drift, 1, seed, offset)
+        for g, w in zip(got, want):
+            assert torch.equal(g, w)
+    with pytest.raises(kg.KappagenError) as e:
+        kg.sample_cells_prepared(ncell, 64, ws[:100], 1, 0, dtype)
+    assert e.value.status == kg.EWORKSPACE
