@@ -48,12 +48,12 @@ NCU_PIPE_PCT = {"f32": {"sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustain
 # rates from kappagen_pipe_probe = profiles/r02_pipe_rates.md), in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a quarter of
 #        the 128-lane FMA rate (probe: 4.1 cycles per warp instruction per scheduler) -> 32 /clk/SM.
-#   f64: the double chain is 87 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.  On sm_100 the FP64
+#   f64: the double chain is 85 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.  On sm_100 the FP64
 #        pipe and the FMA-heavy pipe (Philox's IMAD.WIDE) overlap only in part; their issue cycles per 32 particles sum
-#        to 87 x 2.03 + 18.2 x 4.14 + 9 x 2 scheduler cycles.
+#        to 85 x 2.03 + 18.2 x 4.14 + 9 x 2 scheduler cycles.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
-            "f64": (87, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
-F64_SHARED_PORT_CYCLES = 87 * 2.03 + 18.2 * 4.14 + 9 * 2.0    # per 32 particles per scheduler: FP64 + IMAD.WIDE + IMAD/MOV
+            "f64": (85, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+F64_SHARED_PORT_CYCLES = 85 * 2.03 + 18.2 * 4.14 + 9 * 2.0    # per 32 particles per scheduler: FP64 + IMAD.WIDE + IMAD/MOV
 TARGETS = {"f32": ("hbm", 0.80), "f64": ("alu", 0.70)}         # BASELINE.json north_star, last sentence
 
 

@@ -32,7 +32,7 @@ struct alignas(16) Coef<double> {
     double k2;     // 2 kappa*
     double b2;     // 2 b
     double theta;  // most probable speed; NaN marks an invalid cell
-    double pad;
+    double theta2; // 2 theta: the chain carries 2V, so that neither V + V nor 2 U2 - 1 costs an instruction
 };
 
 // The float chain returns 2V = sqrt(num/den) with
@@ -119,7 +119,7 @@ KAPPAGEN_HD inline Coef<double> make_coef_f64(const TableIParams<F>& P, F theta)
     C.k2 = (double)(F(2.0) * P.kstar);
     C.b2 = (double)(F(2.0) * P.b);
     C.theta = (double)theta;
-    C.pad = 0.0;
+    C.theta2 = (double)(F(2.0) * theta);
     return C;
 }
 

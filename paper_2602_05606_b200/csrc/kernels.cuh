@@ -377,7 +377,7 @@ __device__ __forceinline__ void rec_velocities(const uint32_t (&w0)[2], const ui
     const ulonglong2 (&q)[6] = r.q;
     Coef<double> C;                                                    // the order of CellRec<double>
     C.s = as_f64(q[0].x); C.a = as_f64(q[0].y); C.ck = as_f64(q[1].x); C.bk4 = as_f64(q[1].y);
-    C.k2 = as_f64(q[2].x); C.b2 = as_f64(q[2].y); C.theta = as_f64(q[3].x); C.pad = 0.0;
+    C.k2 = as_f64(q[2].x); C.b2 = as_f64(q[2].y); C.theta = as_f64(q[3].x); C.theta2 = as_f64(q[3].y);
 #pragma unroll
     for (int e = 0; e < 2; ++e)
         velocity_f64<false, true>(w0[e], w1[e], w2[e], 0u, C, ox[e], oy[e], oz[e], as_f64(q[4].x), as_f64(q[4].y), as_f64(q[5].x));
@@ -519,7 +519,7 @@ __device__ __forceinline__ void group_speeds(uint64_t g0, const PhiloxKeys& K, c
     uint32_t w0[2], w1[2], w2[2], w3[2];
     group_words<2>(g0, K, w0, w1, w2, w3);
 #pragma unroll
-    for (int e = 0; e < 2; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
+    for (int e = 0; e < 2; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C, C.theta);
 }
 // Speeds of one group of a whole tile (words through tile_group_words, as in sample_kernel).
 template <bool U64, typename T, int G>
@@ -532,7 +532,7 @@ __device__ __forceinline__ void group_speeds_tile(uint32_t lo_first, uint64_t q_
         for (int e = 0; e < G; e += 2) up2(speed2_f32x2<U64>(w0[e], w0[e + 1], w3[e], w3[e + 1], C), s[e], s[e + 1]);
     } else {
 #pragma unroll
-        for (int e = 0; e < G; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C);
+        for (int e = 0; e < G; ++e) s[e] = speed_f64<U64>(w0[e], w3[e], C, C.theta);
     }
 }
 __device__ __forceinline__ int bin_of(float s, float inv) { return __float2int_rz(s * inv); }     // saturating

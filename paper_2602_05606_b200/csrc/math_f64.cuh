@@ -11,7 +11,7 @@
 //   azimuth: quarter-turn reduction on the integer word, polynomials on |angle| <= pi/4
 // No data-dependent branch: selects only ("no loops or conditional statements").
 //
-// Written for the FP64 pipe of sm_100 (64 DFMA/clk/SM): 87 FP64 instructions per particle instead of
+// Written for the FP64 pipe of sm_100 (64 DFMA/clk/SM): 85 FP64 instructions per particle instead of
 // libdevice's ~200, and no divergent slow paths.  On sm_100 the FP64 pipe and the FMA-heavy pipe (IMAD,
 // IMAD.WIDE, IMAD.MOV) do not overlap in time (profiles/r02_pipe_rates.md), so every instruction of either
 // kind counts against the same budget; the choices below follow from that.
@@ -111,7 +111,7 @@ __device__ __forceinline__ double sqrt3_f64(double z) {
 }
 
 template <bool U64 = false>
-__device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef<double>& C) {
+__device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef<double>& C, double scale) {   // scale sqrt(x)
     double u1, t1;
     float useed;                                                                 // 2^32 U1 for the fp32 seed
     if (U64) {
@@ -149,14 +149,14 @@ __device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef
     const double num = (k == 0) ? -(p * D) : Nk - D;
     const double f = num * rcp3_f64(Nk + D);
     const double z = f * f;
-    double P = 0x1.9d7eab5747345p-4;                                             // atanh(sqrt z)/sqrt z, degree 5: 1.9e-13
-    P = fma(P, z, 0x1.c530318164389p-4);
-    P = fma(P, z, 0x1.2497875fa7cb3p-3);
-    P = fma(P, z, 0x1.99998cbcc9384p-3);
-    P = fma(P, z, 0x1.5555555b16753p-2);
-    P = fma(P, z, 0x1.ffffffffff957p-1);
+    double P = 0x1.9d7eab5747345p-3;                                             // 2 atanh(sqrt z)/sqrt z, degree 5: 1.9e-13
+    P = fma(P, z, 0x1.c530318164389p-3);                                         // (the fitted coefficients, doubled: exact)
+    P = fma(P, z, 0x1.2497875fa7cb3p-2);
+    P = fma(P, z, 0x1.99998cbcc9384p-2);
+    P = fma(P, z, 0x1.5555555b16753p-1);
+    P = fma(P, z, 0x1.ffffffffff957p+0);
     const F64Tables& Tb = f64_tables();
-    const double lnS = fma(f + f, P, Tb.neg_k_ln2[-k]);                          // k ln2 + 2 f P
+    const double lnS = fma(f, P, Tb.neg_k_ln2[-k]);                              // k ln2 + 2 f P(z): P holds 2 P
     // Y = expm1(M), M = -ln(S)/kappa* >= 0:  M = n ln2 + rho,  Y = 2^n (rho Q(rho)) + (2^n - 1)
     const double M = -lnS * C.s;
     const double nb = fma(M, 0x1.71547652b82fep+0, 0x1.8p52);                    // n = rint(M log2 e) in the low word
@@ -181,7 +181,7 @@ __device__ __forceinline__ double speed_f64(uint32_t w0, uint32_t w3, const Coef
     const bool pos = A >= 0.0;
     const double nm = pos ? C.k2 * Y : T;
     const double dn = pos ? T : C.b2;
-    return C.theta * (nm * rsqrt3_f64(nm * dn));
+    return scale * (nm * rsqrt3_f64(nm * dn));
 }
 
 // DRIFT: the cell's drift as the addend of the last multiply (one rounding), as in velocity_f32.
@@ -189,11 +189,11 @@ template <bool U64 = false, bool DRIFT = false>
 __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3,
                                              const Coef<double>& C, double& vx, double& vy, double& vz,
                                              double dx = 0.0, double dy = 0.0, double dz = 0.0) {
-    const double V = speed_f64<U64>(w0, w3, C);
+    const double V2 = speed_f64<U64>(w0, w3, C, C.theta2);                       // 2V: the factor 2 of Table I lines 9-10
     const double x2 = u32_unit(w1);
     const double u2 = x2 - (1.0 - 0x1p-33);                                      // U2, exact
     const double t2 = (2.0 - 0x1p-33) - x2;                                      // 1 - U2, exact
-    const double mu = u2 - t2;                                                   // 2 U2 - 1, exact
+    const double muh = x2 - (1.5 - 0x1p-33);                                     // U2 - 1/2 = (2 U2 - 1)/2, exact
     const double zz = u2 * t2;
     const double sth = sqrt3_f64(zz);                                            // sqrt(U2 (1-U2)); the 2 goes into Vs
     // 2 pi U3 = (pi/2)(k + q): k = nearest quarter turn, q = ((int32)(w2 << 2) + 2)/2^32 in (-1/2, 1/2)
@@ -219,13 +219,13 @@ __device__ __forceinline__ void velocity_f64(uint32_t w0, uint32_t w1, uint32_t 
     // signs: sin < 0 for k = 2,3 (bit 31 of wq); cos < 0 for k = 1,2 (bit 31 of wq + 2^30)
     const double cphi = __hiloint2double(__double2hiint(c0) ^ (int)((wq + 0x40000000u) & 0x80000000u), __double2loint(c0));
     const double sphi = __hiloint2double(__double2hiint(s0) ^ (int)(wq & 0x80000000u), __double2loint(s0));
-    const double Vs = (V + V) * sth;
+    const double Vs = V2 * sth;
     if (DRIFT) {
-        vx = fma(V, mu, dx);
+        vx = fma(V2, muh, dx);
         vy = fma(Vs, cphi, dy);
         vz = fma(Vs, sphi, dz);
     } else {
-        vx = V * mu;
+        vx = V2 * muh;
         vy = Vs * cphi;
         vz = Vs * sphi;
     }
