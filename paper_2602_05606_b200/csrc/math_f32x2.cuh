@@ -33,6 +33,21 @@ __device__ __forceinline__ Coef2 splat_coef(const Coef<float>& C) {
                  splat2(C.th4), splat2(C.theta)};
 }
 
+// Selects as predicated arithmetic on one half of a pair: "if the chain is on its MUFU side, overwrite the polynomial
+// side's value" -- the product / sum is formed by a predicated scalar instruction (as many FMA-pipe cycles as the packed
+// one it replaces) and the two FSELs per pair (ALU pipe) disappear.  .rn: no contraction, same bits as the packed
+// and the scalar chain.  The comparisons are the unordered complements of the scalar chain's (NaN takes the same side).
+__device__ __forceinline__ void mul_if_geu(float& dst, float x, float bound, float a, float b) {
+    asm("{ .reg .pred q; setp.geu.f32 q, %1, %2; @q mul.rn.f32 %0, %3, %4; }" : "+f"(dst) : "f"(x), "f"(bound), "f"(a), "f"(b));
+}
+__device__ __forceinline__ void add_if_geu(float& dst, float x, float bound, float a, float b) {
+    asm("{ .reg .pred q; setp.geu.f32 q, %1, %2; @q add.rn.f32 %0, %3, %4; }" : "+f"(dst) : "f"(x), "f"(bound), "f"(a), "f"(b));
+}
+__device__ __forceinline__ void mul_mov_if_ltu(float& num, float& den, float x, float a, float b, float c) {   // x < 0 or NaN
+    asm("{ .reg .pred q; setp.ltu.f32 q, %2, 0f00000000; @q mul.rn.f32 %0, %3, %4; @q mov.f32 %1, %5; }"
+        : "+f"(num), "+f"(den) : "f"(x), "f"(a), "f"(b), "f"(c));
+}
+
 // 2V for two particles (see speed2_f32).
 template <bool U64>
 __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32_t w3a, uint32_t w3b, const Coef2& C) {
@@ -52,33 +67,37 @@ __device__ __forceinline__ f32x2 speed2_f32x2(uint32_t w0a, uint32_t w0b, uint32
     G = fma2(G, p, splat2(0x1.71565ep-1f));
     G = fma2(G, p, splat2(0x1.715476p+0f));
     const f32x2 m_small = mul2(mul2(p, C.s), G);
-    const f32x2 m_large = mul2(KG_MAP2(mufu_lg2, S), C.ms);
-    float pa, pb, msa, msb, mla, mlb;
-    up2(p, pa, pb); up2(m_small, msa, msb); up2(m_large, mla, mlb);
-    const float ma = (pa < 0.25f) ? msa : mla, mb = (pb < 0.25f) ? msb : mlb;
+    float pa, pb, ma, mb;
+    up2(p, pa, pb);
+    {
+        float Sa, Sb, msa, msb;
+        up2(S, Sa, Sb); up2(C.ms, msa, msb); up2(m_small, ma, mb);
+        mul_if_geu(ma, pa, 0.25f, mufu_lg2(Sa), msa);
+        mul_if_geu(mb, pb, 0.25f, mufu_lg2(Sb), msb);
+    }
     const f32x2 m = pk2(ma, mb);
     f32x2 R = fma2(splat2(0x1.945094p-10f), m, splat2(0x1.3817fcp-7f));
     R = fma2(R, m, splat2(0x1.c6d414p-5f));
     R = fma2(R, m, splat2(0x1.ebfb52p-3f));
     R = fma2(R, m, splat2(0x1.62e43p-1f));
     const f32x2 y_small = mul2(m, R);
-    const f32x2 y_large = add2(KG_MAP2(mufu_ex2, m), splat2(-1.0f));
-    float ysa, ysb, yla, ylb;
-    up2(y_small, ysa, ysb); up2(y_large, yla, ylb);
-    const f32x2 Y = pk2((ma < 0.5f) ? ysa : yla, (mb < 0.5f) ? ysb : ylb);
+    float Ya, Yb;
+    up2(y_small, Ya, Yb);
+    add_if_geu(Ya, ma, 0.5f, mufu_ex2(ma), -1.0f);
+    add_if_geu(Yb, mb, 0.5f, mufu_ex2(mb), -1.0f);
+    const f32x2 Y = pk2(Ya, Yb);
     const f32x2 A = fma2(Y, C.mck, C.a);
     const f32x2 D = KG_MAP2(mufu_sqrt, fma2(A, A, mul2(Y, C.bk4)));
     float Aa, Ab, Da, Db;
     up2(A, Aa, Ab); up2(D, Da, Db);
     const float Ta = fabsf(Aa) + Da, Tb = fabsf(Ab) + Db;
-    const f32x2 n_pos = mul2(Y, C.k2), n_neg = mul2(pk2(Ta, Tb), C.th4);
-    float npa, npb, nna, nnb;
-    up2(n_pos, npa, npb); up2(n_neg, nna, nnb);
-    const bool posa = Aa >= 0.0f, posb = Ab >= 0.0f;
-    const f32x2 num = pk2(posa ? npa : nna, posb ? npb : nnb);
     float b2a, b2b;
     up2(C.b2, b2a, b2b);
-    const f32x2 den = pk2(posa ? Ta : b2a, posb ? Tb : b2b);
+    float na, nb, da = Ta, db = Tb, t4a, t4b;
+    up2(mul2(Y, C.k2), na, nb); up2(C.th4, t4a, t4b);
+    mul_mov_if_ltu(na, da, Aa, Ta, t4a, b2a);
+    mul_mov_if_ltu(nb, db, Ab, Tb, t4b, b2b);
+    const f32x2 num = pk2(na, nb), den = pk2(da, db);
     return mul2(num, KG_MAP2(mufu_rsq, mul2(num, den)));
 }
 
