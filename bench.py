@@ -36,14 +36,14 @@ N_SM = 148
 # ncu figures of one sample_kernel launch at 2^28 particles (dram__bytes_read.sum + dram__bytes_write.sum, busy
 # fraction of the pipes), copied from the `ncu --set full` captures summarised in profiles/r02_kernels.md.  They are
 # NOT measured by this run: the line prints them under "ncu" with their source so that nobody takes them for it.
-NCU_CAPTURE = {"from": "profiles/r02_kernels.md", "kernels_as_of_commit": "float sampler as of 77e407b, double sampler as of the 85-instruction chain (round 2, final)",
+NCU_CAPTURE = {"from": "profiles/r02_kernels.md", "kernels_as_of_commit": "006351f (round 2, final kernels)",
                "note": "copied from an ncu --set full capture, not measured by this run"}
-NCU_TRAFFIC_BYTES = {"f32": 3161219400, "f64": 6382977944}       # dram__bytes_read.sum + dram__bytes_write.sum per launch
-NCU_PIPE_PCT = {"f32": {"sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 76.0,
-                        "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active": 54.8,
-                        "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active": 40.4},
+NCU_TRAFFIC_BYTES = {"f32": 3161401296, "f64": 6383825960}       # dram__bytes_read.sum + dram__bytes_write.sum per launch
+NCU_PIPE_PCT = {"f32": {"sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 74.8,
+                        "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active": 53.9,
+                        "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active": 41.6},
                 "f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.6,
-                        "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 32.8}}
+                        "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 32.7}}
 # Algorithmic work per particle on the arithmetic pipes (instruction counts from cuobjdump -sass,
 # rates from kappagen_pipe_probe = profiles/r02_pipe_rates.md), in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a quarter of
