@@ -15,7 +15,8 @@
  * Conventions for every call:
  *  - "device" pointers are CUDA device memory owned by the caller (e.g. torch tensor.data_ptr());
  *    "host" pointers are ordinary host memory.  The library keeps no state and no RNG state,
- *    and allocates nothing that outlives a call.
+ *    and allocates nothing that outlives a call (kappagen_sample_cells_static keeps its scratch in
+ *    a fixed array inside the library image instead: see there).
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device-buffer
  *    calls enqueue on `stream` and return without synchronising; argument errors are returned
  *    at once, asynchronous CUDA errors surface at the caller's next synchronisation.  They
@@ -84,6 +85,34 @@ int kappagen_sample_cells(int64_t ncell, int32_t ppc, const void* kappa, const v
                           int dtype, void* vx, void* vy, void* vz,
                           void* workspace, size_t workspace_bytes, void* stream);
 size_t kappagen_cells_workspace_bytes(int64_t ncell, int dtype);
+
+/* kappagen_sample_cells for callers that cannot hand over a workspace because they cannot get device memory at
+ * all: a particle-injection routine called every time step inside a simulation whose framework took the whole
+ * GPU into its own pool at start-up and forbids cudaMalloc afterwards (it stalls every stream of the device and
+ * may simply fail once the pool holds everything), or a plug-in that is given output arrays but no handle to
+ * that pool.  This call allocates nothing -- no cudaMalloc, no cudaFree, no library routine that allocates --
+ * and the caller passes only inputs and outputs.  The per-cell records that kappagen_sample_cells keeps in
+ * `workspace` are kept instead in an array of KAPPAGEN_STATIC_SCRATCH_BYTES bytes built into the library's
+ * device code.  That array costs its size on every GPU that loads libkappagen, from load until the process
+ * ends, whether or not this call is ever made; hence the modest limit:
+ *     ncell <= KAPPAGEN_STATIC_SCRATCH_BYTES / 48 = 65536 cells per call (float), / 96 = 32768 (double).
+ * More cells: KAPPAGEN_EWORKSPACE, reported before anything touches the device, with the limit in
+ * kappagen_last_error(); split the call (cells c0 .. c1-1 on their own: kappa + c0, theta + c0, the planes
+ * + c0*ppc and offset + c0*ppc give the same particles) or use kappagen_sample_cells.
+ *  - First call on each device: it asks the CUDA runtime where the array lives on the current device and
+ *    remembers the answer (per device, thread-safe).  Make that first call with the device you mean to use
+ *    current, in ordinary execution, before any stream capture is begun.  Later calls only launch kernels.
+ *  - One array per GPU, shared by every call from every thread and stream.  Calls that can run on the GPU at the
+ *    same time (different streams, or the same stream from two unsynchronised threads) overwrite each other's
+ *    records and produce garbage: order them on one stream, or by events.  The array keeps the last call's
+ *    records; this call rewrites every record it reads, so nothing has to be cleared and nothing leaks from one
+ *    call into the next.
+ * Values are bit-identical to kappagen_sample_cells with the same arguments; all other arguments, the NaN
+ * convention for invalid cells and the other error codes are as there. */
+#define KAPPAGEN_STATIC_SCRATCH_BYTES 3145728 /* 3 MiB */
+int kappagen_sample_cells_static(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                 const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                 int dtype, void* vx, void* vy, void* vz, void* stream);
 
 /* The two halves of kappagen_sample_cells as calls of their own: "The first four lines [of Table I] are required
  * only once".  kappagen_cells_prepare fills the workspace with the per-cell records (Table I

@@ -4,6 +4,8 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <mutex>
+
 #include <cuda_runtime.h>
 
 #include "../../include/kappagen.h"
@@ -295,6 +297,67 @@ extern "C" int kappagen_sample_cells_moments(int64_t ncell, int32_t ppc, const v
                                              size_t workspace_bytes, void* stream) {
     return cells_impl("kappagen_sample_cells_moments", ncell, ppc, kappa, theta, drift, drift_stride, seed, offset, dtype, vx,
                       vy, vz, moments, true, workspace, workspace_bytes, stream);
+}
+
+// ---- kappagen_sample_cells_static: kappagen_sample_cells for callers that have no device memory to hand over as
+// workspace and may not ask the driver for any (see include/kappagen.h).  The per-cell records live in the array
+// below, which is part of the library's device image: it is reserved on every GPU that loads libkappagen and stays
+// reserved until the process exits, so it is kept small.  The kernels are the ones kappagen_sample_cells launches;
+// only the place the records are kept differs.
+static __device__ __align__(256) unsigned char g_static_cells_scratch[KAPPAGEN_STATIC_SCRATCH_BYTES];
+
+// Where g_static_cells_scratch sits on the CURRENT device.  On the host the array's name is only a handle for the
+// runtime, not somewhere a kernel can write: the address a kernel may use comes from cudaGetSymbolAddress, differs
+// from GPU to GPU, and is looked up once per device (under a lock: two host threads may arrive here first together).
+static int static_cells_scratch(const char* fn, void** out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static void* addr[kMaxDev] = {};
+    int dev = -1;
+    KG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDev) {
+        set_error("%s: device ordinal %d is outside the %d this call keeps an address for", fn, dev, kMaxDev);
+        return KAPPAGEN_ECUDA;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (addr[dev] == nullptr) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_cells_scratch);
+        if (e != cudaSuccess || p == nullptr) {
+            set_error("%s: cudaGetSymbolAddress of the built-in scratch failed on device %d: %s", fn, dev, cudaGetErrorString(e));
+            return KAPPAGEN_ECUDA;
+        }
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_sample_cells_static(int64_t ncell, int32_t ppc, const void* kappa, const void* theta,
+                                            const void* drift, int64_t drift_stride, uint64_t seed, uint64_t offset,
+                                            int dtype, void* vx, void* vy, void* vz, void* stream) {
+    const char* fn = "kappagen_sample_cells_static";
+    if (dtype != KAPPAGEN_F32 && dtype != KAPPAGEN_F64) {
+        set_error("%s: dtype %d is neither KAPPAGEN_F32 nor KAPPAGEN_F64", fn, dtype);
+        return KAPPAGEN_EINVAL;
+    }
+    const size_t rec = dtype == KAPPAGEN_F32 ? sizeof(CellRec<float>) : sizeof(CellRec<double>);
+    const int64_t most = (int64_t)(KAPPAGEN_STATIC_SCRATCH_BYTES / rec);
+    if (ncell > most) {                                               // before anything touches the device
+        set_error("%s: %lld cells need %zu bytes of per-cell records, the built-in scratch holds %d bytes (at most %lld cells "
+                  "of this dtype per call): split the call, or use kappagen_sample_cells with a workspace of your own",
+                  fn, (long long)ncell, (size_t)ncell * rec, (int)KAPPAGEN_STATIC_SCRATCH_BYTES, (long long)most);
+        return KAPPAGEN_EWORKSPACE;
+    }
+    void* scratch = nullptr;
+    if (ncell > 0 && ppc > 0) {                                       // nothing to launch otherwise: cells_impl only checks
+        const int rc = static_cells_scratch(fn, &scratch);
+        if (rc != KAPPAGEN_OK) return rc;
+    }
+    // every record of cells 0 .. ncell-1 is rewritten in full by the pre-kernel before the sampler reads it, so what an
+    // earlier call left in the array is never seen and nothing needs clearing
+    return cells_impl(fn, ncell, ppc, kappa, theta, drift, drift_stride, seed, offset, dtype, vx, vy, vz, nullptr, false,
+                      scratch, KAPPAGEN_STATIC_SCRATCH_BYTES, stream);
 }
 
 extern "C" int kappagen_baseline_mt(int64_t n, double kappa, double theta, uint64_t seed, uint64_t offset, int dtype,

@@ -50,6 +50,7 @@ def lib() -> ctypes.CDLL:
         L.kappagen_speed_histogram.argtypes = [i64, f64, u64, u64, ci, ctypes.c_uint32, f64, i32, vp, vp]
         L.kappagen_relative_entropy.argtypes = [vp, i32, f64, f64, f64, ci, ctypes.POINTER(ctypes.c_double)]
         L.kappagen_sample_cells.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, sz, vp]
+        L.kappagen_sample_cells_static.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp]
         L.kappagen_sample_cells_moments.argtypes = [i64, i32, vp, vp, vp, i64, u64, u64, ci, vp, vp, vp, vp, vp, sz, vp]
         L.kappagen_cells_prepare.argtypes = [i64, vp, vp, vp, i64, ci, vp, sz, vp]
         L.kappagen_sample_cells_prepared.argtypes = [i64, i32, u64, u64, ci, vp, vp, vp, vp, sz, vp]
@@ -71,7 +72,7 @@ def lib() -> ctypes.CDLL:
         L.kappagen_params.argtypes = [f64, dp, dp, dp, dp]
         L.kappagen_last_error.restype = ctypes.c_char_p
         for name in ("kappagen_speed_histogram", "kappagen_relative_entropy", "kappagen_sample", "kappagen_sample_flags", "kappagen_words4", "kappagen_velocity_of_words_u64",
-                     "kappagen_sample_cells", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
+                     "kappagen_sample_cells", "kappagen_sample_cells_static", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version",
                      "kappagen_words_tile", "kappagen_velocity_of_words_tile", "kappagen_sample_host_ws",
                      "kappagen_load_cells", "kappagen_cells_prepare", "kappagen_sample_cells_prepared", "kappagen_philox_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
@@ -203,6 +204,26 @@ def sample_cells(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None,
                                        drift.data_ptr() if drift is not None else None, drift_stride, seed, offset,
                                        code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), workspace.data_ptr(),
                                        workspace.numel() * workspace.element_size(), _stream(stream)))
+    return vx, vy, vz
+
+
+STATIC_SCRATCH_BYTES = 3 << 20      # KAPPAGEN_STATIC_SCRATCH_BYTES of include/kappagen.h
+
+
+def sample_cells_static(ppc: int, kappa: torch.Tensor, theta: torch.Tensor, drift=None, drift_stride: int = 0,
+                        seed: int = 0, offset: int = 0, out=None, stream=None):
+    """kappagen_sample_cells_static: sample_cells for code that may not allocate device memory (a routine inside a
+    simulation whose framework owns the whole GPU through its own pool and bans cudaMalloc after start-up).  No
+    workspace argument: the per-cell records go to a 3 MiB array built into the library, so one call takes at most
+    65536 float / 32768 double cells (more raises KappagenError with EWORKSPACE), calls that overlap on the GPU
+    corrupt each other, and the first call on a device should be made outside stream capture.  Pass `out` (three
+    preallocated planes) to keep this wrapper from allocating them with torch.  Same values as sample_cells."""
+    code, ncell = _cell_inputs(ppc, kappa, theta, drift, drift_stride)
+    vx, vy, vz = _planes(ncell * ppc, code, out, kappa.device)
+    _same_device(kappa, vx)
+    _check(lib().kappagen_sample_cells_static(ncell, ppc, kappa.data_ptr(), theta.data_ptr(),
+                                              drift.data_ptr() if drift is not None else None, drift_stride, seed,
+                                              offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
     return vx, vy, vz
 
 
