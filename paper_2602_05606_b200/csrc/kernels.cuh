@@ -259,8 +259,9 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
     const double ks = ok ? kap - 0.5 : 1.0;
     const double lnB = lgamma(1.5) + lgamma(ks) - lgamma(ks + 1.5);   // ln B(3/2, kappa*)
     const TableIParams<double> P = table1_params<double>(ok ? kap : 2.5, lnB, c_approx_f64(ok ? kap : 2.5));
-    Coef<T> C = cell_coef<T>(P, th);
-    if (!ok) C.theta = (T)nan("");                                    // whole cell becomes NaN
+    // an invalid cell becomes NaN in all its particles: poison theta at the source, so that every constant derived
+    // from it (theta for float, theta and 2 theta for double) carries the NaN into the chain
+    const Coef<T> C = cell_coef<T>(P, ok ? th : nan(""));
     T dx = T(0), dy = T(0), dz = T(0);
     if (drift != nullptr) {
         const T* d = drift + 3 * cell * drift_stride;
@@ -275,6 +276,13 @@ cell_coef_kernel(int64_t ncell, const T* __restrict__ kappa, const T* __restrict
 __device__ __forceinline__ int64_t cell_of(int64_t i, uint32_t ppc, uint64_t magic) {
     if (magic < 64ull) return i >> (int)magic;
     return magic != ~0ull ? (int64_t)__umul64hi((uint64_t)i, magic) : i / (int64_t)ppc;
+}
+
+// Whole cells between a tile's first particle and the particle o places after the first particle's cell began
+// (o < tile + ppc).  magic32 = ceil(2^32 / ppc) where the launcher found it exact for these o; magic32 == 0 means
+// ppc >= tile (the launcher's cells_magics() guarantees it), so o < 2 ppc and the answer is 0 or 1.
+__device__ __forceinline__ uint32_t cells_ahead(uint32_t o, uint32_t ppc, uint32_t magic32) {
+    return magic32 != 0u ? __umulhi(o, magic32) : (uint32_t)(o >= ppc);
 }
 
 // How the fused moments (kappagen_sample_cells_moments) leave the kernel.  All sums are in T.
@@ -395,7 +403,7 @@ __device__ __forceinline__ void rec_velocity(uint32_t w0, uint32_t w1, uint32_t 
 // code as the uniform sampler; a group that straddles a cell boundary takes the per-particle path.
 // Whole tiles (in range, inside one 2^32 block of counters) run in one straight line, as in the uniform sampler;
 // a group finds its cell with one 32-bit multiply-high from its offset inside the tile (magic32 = ceil(2^32 / ppc),
-// exact for those offsets; 0 switches the path off) and the tile's first cell, which the block carries from tile to
+// exact for those offsets; 0: ppc >= tile, one compare instead -- cells_ahead()) and the tile's first cell, which the block carries from tile to
 // tile by addition.
 // STORE: write the velocity planes.  MOM: also reduce (sum vx, sum vy, sum vz, sum |v|^2) per cell into
 // mom[ncell][4] -- the loader fused with its first consumer: with STORE = false
@@ -418,7 +426,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, u
     const uint32_t drem = (uint32_t)(stride - dcell * (int64_t)ppc);
     for (; base < n; base += stride) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (VEC && whole_groups && magic32 != 0u && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
+        if (VEC && whole_groups && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             // the straight-line tile of the uniform sampler (one Philox head; float: round-1 products by constant additions)
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
@@ -428,7 +436,7 @@ sample_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, u
             RecRegs<T> rec[kGroups];
 #pragma unroll
             for (int j = 0; j < kGroups; ++j) {
-                cell[j] = cell_first + (int64_t)__umulhi(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, magic32);
+                cell[j] = cell_first + (int64_t)cells_ahead(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, ppc, magic32);
                 load_rec(W, cell[j], rec[j]);
             }
 #pragma unroll
