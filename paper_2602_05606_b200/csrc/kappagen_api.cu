@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <atomic>
 #include <mutex>
 
 #include <cuda_runtime.h>
@@ -147,6 +148,26 @@ static int launch_cells_as(int64_t n, int32_t ppc, uint64_t magic, uint32_t magi
     return KAPPAGEN_OK;
 }
 
+// The two constants that replace the division by ppc in the per-cell kernels (sample_cells_kernel, load_cells_kernel).
+//  magic  : cell_of(): a shift count when ppc is a power of two; else floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1), exact
+//           for every i with i * ppc < 2^64 (i < n; the value is >= 2^32 > 64 for every ppc < 2^31); else ~0: the plain
+//           64-bit division.
+//  magic32: inside a tile, floor(o/ppc) = mulhi32(o, ceil(2^32/ppc)), exact while o * ppc < 2^32 (o < tile + ppc).
+//           0 = no such constant: ppc == 1, or ppc so large ((tile + ppc) * ppc >= 2^32, i.e. ppc > 6.4e4 >= tile) that a
+//           tile touches at most two cells and the kernels compare instead (cells_ahead()).
+static void cells_magics(int64_t n, int32_t ppc, int64_t tile, uint64_t* magic, uint32_t* magic32) {
+    const uint64_t up = (uint64_t)ppc;
+    *magic = ~0ull;
+    if ((up & (up - 1)) == 0) {
+        *magic = 0;
+        while ((1ull << *magic) < up) ++*magic;
+    } else if ((uint64_t)n <= (~0ull) / up) {
+        *magic = (~0ull) / up + 1;
+    }
+    *magic32 = 0;
+    if (up >= 2 && ((uint64_t)tile + up) * up < (1ull << 32)) *magic32 = (uint32_t)(((1ull << 32) + up - 1) / up);
+}
+
 // store: write the planes; mom != nullptr: fused per-cell moments (at least one of the two).
 template <typename T>
 static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* theta, const T* drift,
@@ -169,19 +190,9 @@ static int launch_cells(int64_t ncell, int32_t ppc, const T* kappa, const T* the
     }
     if (!sample) return KAPPAGEN_OK;
     const int64_t n = ncell * (int64_t)ppc;
-    // cell_of(): a shift when ppc is a power of two; else floor(i/ppc) = mulhi64(i, floor(2^64/ppc) + 1), exact for
-    // every i with i * ppc < 2^64 (i < n); else (~0) the plain 64-bit division
-    const uint64_t up = (uint64_t)ppc;
-    uint64_t magic = ~0ull;
-    if ((up & (up - 1)) == 0) {
-        magic = 0;
-        while ((1ull << magic) < up) ++magic;
-    } else if ((uint64_t)n <= (~0ull) / up) {
-        magic = (~0ull) / up + 1;                           // >= 2^32 > 64 for every ppc < 2^31
-    }
-    // inside a tile: floor(o/ppc) = mulhi32(o, ceil(2^32/ppc)), exact while o * ppc < 2^32 (o < tile + ppc); 0 = not used
-    uint32_t magic32 = 0;
-    if (up >= 2 && ((uint64_t)tile + up) * up < (1ull << 32)) magic32 = (uint32_t)(((1ull << 32) + up - 1) / up);
+    uint64_t magic;
+    uint32_t magic32;
+    cells_magics(n, ppc, tile, &magic, &magic32);
 #define KG_CELLS(V, S, M) launch_cells_as<T, V, S, M>(n, ppc, magic, magic32, offset, K, W, vx, vy, vz, mom, mode, lanes, st)
     if (mom == nullptr) return vec ? KG_CELLS(true, true, false) : KG_CELLS(false, true, false);
     if (!store) return KG_CELLS(true, false, true);
@@ -761,24 +772,22 @@ extern "C" int kappagen_sample_cells_prepared(int64_t ncell, int32_t ppc, uint64
 }
 
 // ---- kappagen_load_cells: per-cell velocities and positions as one AoS record per particle (load_cells.cuh)
-static void cells_magics(int64_t n, int32_t ppc, int64_t tile, uint64_t* magic, uint32_t* magic32) {
-    const uint64_t up = (uint64_t)ppc;
-    *magic = ~0ull;
-    if ((up & (up - 1)) == 0) {
-        *magic = 0;
-        while ((1ull << *magic) < up) ++*magic;
-    } else if ((uint64_t)n <= (~0ull) / up) {
-        *magic = (~0ull) / up + 1;
-    }
-    *magic32 = 0;
-    if (up >= 2 && ((uint64_t)tile + up) * up < (1ull << 32)) *magic32 = (uint32_t)(((1ull << 32) + up - 1) / up);
-}
-
 template <typename T, bool HASW>
 static int launch_load_as(int64_t n, int32_t ppc, uint64_t offset, const PhiloxKeys& K, const CellRec<T>* W, const T* weight,
                           int64_t cell_base, T* out, cudaStream_t st) {
     constexpr int64_t tile = (int64_t)kThreads * (16 / sizeof(T)) * kGroups;
-    KG_CUDA(cudaFuncSetAttribute(load_cells_kernel<T, HASW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLoadSmemBytes));
+    {   // the opt-in to the kernel's dynamic shared memory is per device and sticks: once per device and instantiation,
+        // not on every launch (small calls are launch-bound)
+        constexpr int kMaxDev = 64;
+        static std::atomic<bool> opted_in[kMaxDev] = {};
+        int dev = 0;
+        KG_CUDA(cudaGetDevice(&dev));
+        const bool cached = dev >= 0 && dev < kMaxDev;
+        if (!cached || !opted_in[dev].load(std::memory_order_acquire)) {
+            KG_CUDA(cudaFuncSetAttribute(load_cells_kernel<T, HASW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLoadSmemBytes));
+            if (cached) opted_in[dev].store(true, std::memory_order_release);
+        }
+    }
     uint64_t magic;
     uint32_t magic32;
     cells_magics(n, ppc, tile, &magic, &magic32);
@@ -899,7 +908,8 @@ extern "C" int kappagen_pipe_probe(int mix, int warps_per_scheduler, int iters, 
         return KAPPAGEN_ENULL;
     }
     static PipeProbeFn table[kPipeMixCount] = {};
-    if (table[0] == nullptr) PipeProbeTable<0>::fill(table);
+    static std::once_flag table_once;                                 // two host threads may make the first call together
+    std::call_once(table_once, [] { PipeProbeTable<0>::fill(table); });
     if (counts) {
         const PipeMix M = kPipeMixes[mix];
         counts[0] = M.wide; counts[1] = M.lop3; counts[2] = M.ffma2; counts[3] = M.mufu; counts[4] = M.dfma; counts[5] = M.imad;
@@ -918,9 +928,17 @@ extern "C" int kappagen_pipe_probe(int mix, int warps_per_scheduler, int iters, 
     }
     int status = KAPPAGEN_OK;
     long long* host = new long long[sms];
-    for (int pass = 0; pass < 2; ++pass) table[mix]<<<sms, threads>>>(iters, 1u, sink, cyc);   // the second pass is timed warm
-    if (cudaMemcpy(host, cyc, (size_t)sms * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
-        set_error("%s: kernel or copy failed: %s", fn, cudaGetErrorString(cudaGetLastError()));
+    cudaError_t launched = cudaSuccess;
+    for (int pass = 0; pass < 2 && launched == cudaSuccess; ++pass) {                           // the second pass is timed warm
+        table[mix]<<<sms, threads>>>(iters, 1u, sink, cyc);
+        launched = cudaGetLastError();
+    }
+    cudaError_t copied = cudaSuccess;
+    if (launched != cudaSuccess) {
+        set_error("%s: launch of mix %d failed: %s", fn, mix, cudaGetErrorString(launched));
+        status = KAPPAGEN_ECUDA;
+    } else if ((copied = cudaMemcpy(host, cyc, (size_t)sms * sizeof(long long), cudaMemcpyDeviceToHost)) != cudaSuccess) {
+        set_error("%s: kernel or copy failed: %s", fn, cudaGetErrorString(copied));
         status = KAPPAGEN_ECUDA;
     } else {
         double mean = 0.0;

@@ -91,7 +91,7 @@ load_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, uin
     const uint32_t drem = (uint32_t)(stride - dcell * (int64_t)ppc);
     for (; base < n; base += stride) {
         const uint64_t g_tile = offset + (uint64_t)base;
-        if (whole_groups && magic32 != 0u && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
+        if (whole_groups && base + kTile <= n && tile_in_one_block(g_tile, kTile)) {
             const PhiloxHead H = philox_head((uint32_t)(g_tile >> 32), K);
             const uint32_t lo_first = (uint32_t)g_tile + threadIdx.x * (uint32_t)G;
             const uint64_t q_first = (uint64_t)kPhiloxM0 * (uint64_t)lo_first;
@@ -102,7 +102,7 @@ load_cells_kernel(int64_t n, uint32_t ppc, uint64_t magic, uint32_t magic32, uin
             T wgts[kGroups];
 #pragma unroll
             for (int j = 0; j < kGroups; ++j) {
-                cells[j] = cell_first + (int64_t)__umulhi(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, magic32);
+                cells[j] = cell_first + (int64_t)cells_ahead(rem_first + (uint32_t)(j * (kThreads * G)) + threadIdx.x * (uint32_t)G, ppc, magic32);
                 load_rec(W, cells[j], recs[j]);
                 wgts[j] = HASW ? __ldg(weight + cells[j]) : T(1);
             }
