@@ -34,16 +34,18 @@ FALLBACK_HBM_GBS = 6650.0              # B200_PROFILING.md fallback when MEASURE
 FALLBACK_SM_MHZ = 1965.0               # B200 maximum SM clock (MEASURED_PEAKS.json sm_max_mhz when present)
 N_SM = 148
 # ncu figures of one sample_kernel launch at 2^28 particles (dram__bytes_read.sum + dram__bytes_write.sum, busy
-# fraction of the pipes), copied from the `ncu --set full` captures summarised in profiles/r02_kernels.md.  They are
-# NOT measured by this run: the line prints them under "ncu" with their source so that nobody takes them for it.
-NCU_CAPTURE = {"from": "profiles/r02_kernels.md", "kernels_as_of_commit": "006351f (round 2, final kernels)",
-               "note": "copied from an ncu --set full capture, not measured by this run"}
-NCU_TRAFFIC_BYTES = {"f32": 3161401296, "f64": 6383825960}       # dram__bytes_read.sum + dram__bytes_write.sum per launch
-NCU_PIPE_PCT = {"f32": {"sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 74.8,
-                        "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active": 53.9,
-                        "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active": 41.6},
-                "f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.6,
-                        "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed": 32.7}}
+# fraction of the pipes) come from the tracked profiles/r03_ncu.json, which names the capture command, the commit the
+# kernels were at and the markdown summary that holds the same numbers.  They are NOT measured by this run: the line
+# prints them under "ncu" with that source so that nobody takes them for it.
+def load_ncu():
+    with open(os.path.join(ROOT, "profiles", "r03_ncu.json")) as f:
+        j = json.load(f)
+    src = dict(j["source"], note="copied from an ncu --set full capture, not measured by this run")
+    return src, {d: j["sample_kernel"][d]["dram_bytes_per_launch"] for d in ("f32", "f64")}, \
+        {d: j["sample_kernel"][d]["pipe_busy_pct"] for d in ("f32", "f64")}
+
+
+NCU_CAPTURE, NCU_TRAFFIC_BYTES, NCU_PIPE_PCT = load_ncu()
 # Algorithmic work per particle on the arithmetic pipes (instruction counts from cuobjdump -sass,
 # rates from kappagen_pipe_probe = profiles/r02_pipe_rates.md), in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a quarter of
@@ -53,8 +55,12 @@ NCU_PIPE_PCT = {"f32": {"sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustain
 #        to 85 x 2.03 + 18.2 x 4.14 + 9 x 2 scheduler cycles.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
             "f64": (85, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
+# What the SASS executes per particle on that pipe: the shared Philox head per tile leaves 18.1 of the 19 algorithmic
+# multiplies (17.1 IMAD.WIDE + 1 IMAD.HI, profiles/r02_fp32_limit.md); the double chain executes its 85.
+ALU_EXECUTED = {"f32": 18.1, "f64": 85.0}
 F64_SHARED_PORT_CYCLES = 85 * 2.03 + 18.2 * 4.14 + 9 * 2.0    # per 32 particles per scheduler: FP64 + IMAD.WIDE + IMAD/MOV
 TARGETS = {"f32": ("hbm", 0.80), "f64": ("alu", 0.70)}         # BASELINE.json north_star, last sentence
+BOUND = {"f32": "alu", "f64": "alu"}                           # the measured limiter of each kernel (ncu pipe figures)
 
 
 def measured_peaks():
@@ -72,8 +78,10 @@ def measured_peaks():
 
 def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None):
     """The roofline object of sample_kernel<dtype> from this run's CUDA-event time per launch.
-    f32: the north_star's figure is the HBM write fraction (12 B per particle against the measured copy peak), so that
-    is `frac`; the pipe that actually binds the kernel is beside it under "pipe".  f64: `frac` is the FP64 pipe."""
+    `bound`/`achieved`/`peak`/`frac` name the pipe that actually limits the kernel (both dtypes: an arithmetic pipe,
+    "alu"): algorithmic pipe operations per second against the pipe's issue rate.  The north_star's own figures stay
+    beside it: `frac_hbm` (HBM write fraction against the measured copy peak) and `target` (f32: 0.80 of HBM, judged on
+    frac_hbm; f64: 0.70 of the FP64 pipe, judged on frac_pipe)."""
     es = 4 if dtype == "f32" else 8
     peak, which, mhz = measured_peaks()
     ops, per_clk, alu_unit, pipe = ALU_WORK[dtype]
@@ -86,17 +94,21 @@ def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None):
            "algorithmic_ops_per_particle": ops,
            "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5, profiles/r02_pipe_rates.md)" % (N_SM, per_clk, mhz)}
     alu["frac"] = alu["achieved"] / alu_peak
+    alu["executed_ops_per_particle"] = ALU_EXECUTED[dtype]
+    alu["frac_executed"] = alu["frac"] * ALU_EXECUTED[dtype] / ops
     kind, goal = TARGETS[dtype]
-    head = dict(hbm) if kind == "hbm" else dict(alu)
-    r = {"bound": kind, "achieved": head["achieved"], "peak": head["peak"], "unit": head["unit"], "frac": head["frac"],
+    judged = hbm["frac"] if kind == "hbm" else alu["frac"]
+    head = dict(hbm) if BOUND[dtype] == "hbm" else dict(alu)
+    r = {"bound": BOUND[dtype], "achieved": head["achieved"], "peak": head["peak"], "unit": head["unit"], "frac": head["frac"],
          "traffic": NCU_TRAFFIC_BYTES[dtype], "kernel": "sample_kernel<%s>" % dtype, "kernel_ms": kern_ms,
          "kernel_ms_min": kern_min, "kernel_ms_max": kern_max, "frac_hbm": hbm["frac"], "frac_pipe": alu["frac"],
-         "hbm": hbm, "pipe": alu, "target": {"kind": kind, "frac": goal, "met": head["frac"] >= goal},
+         "hbm": hbm, "pipe": alu, "target": {"kind": kind, "frac": goal, "achieved_frac": judged, "met": judged >= goal},
          "ncu": {"source": NCU_CAPTURE, "dram_bytes_per_launch": NCU_TRAFFIC_BYTES[dtype], "pipe_busy_pct": NCU_PIPE_PCT[dtype]}}
     if dtype == "f32":
         r["bound_note"] = ("compute-bound: the FMA-heavy pipe (Philox's IMAD.WIDE + packed FMA) limits the kernel, not HBM; "
-                           "frac is the HBM write fraction the north_star asks for, frac_pipe the multiply pipe, "
-                           "frac_of_ceiling the same kernel with steps S2-S5 stripped (kappagen_philox_planes)")
+                           "frac = frac_pipe is the multiply pipe (19 algorithmic multiplies per particle; frac_executed "
+                           "counts the 18.1 the SASS issues), frac_hbm the HBM write fraction the north_star asks for "
+                           "(target), frac_of_ceiling the same kernel with steps S2-S5 stripped (kappagen_philox_planes)")
     else:
         cyc = kern_ms * 1e-3 * mhz * 1e6 * N_SM * 4 * 32 / n           # scheduler cycles per 32 particles
         r["shared_port"] = {"cycles_per_32_particles": cyc, "fp64_plus_fmaheavy_cycles": F64_SHARED_PORT_CYCLES,
@@ -125,6 +137,16 @@ def parse_args():
     ap.add_argument("--sweep", action="store_true",
                     help="also time kappagen_sample over 1e6 ... 2^30 particles and kappa 1.6 ... 10 (extras.sweep)")
     return ap.parse_args()
+
+
+def reference_config_dict():
+    """What the --impl reference arm runs: a bounded sample of the same workload on the host, in the oracle's arithmetic."""
+    return {"workload": "bounded sample of BASELINE.json configs[2]: %d particles per step (not 2^28), kappa=2.0, theta=0.1, "
+                        "seed=42, oracle.sample on one host thread, long double arithmetic returned as f64 planes, "
+                        "Philox offset advances by %d per step" % (REF_SAMPLE, REF_SAMPLE),
+            "particles_per_step_per_gpu": REF_SAMPLE, "kappa": KAPPA, "theta": THETA, "seed": SEED,
+            "parallelism": "none: rank 0's host cores only, no GPU", "arithmetic": "long double -> f64",
+            "full_workload_particles_per_step": N_STEP}
 
 
 def config_dict(dtype, world):
@@ -178,7 +200,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": config_dict(args.dtype, 1),
+        "config": reference_config_dict(),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
