@@ -159,5 +159,14 @@ def test_baseline_mt_samples_the_exact_kappa_distribution(kappa, dtype):
     for q in range(3):                                       # direction cosines: mean 0, variance 1/3
         c = (v[q].double() / torch.sqrt(torch.tensor(x, device="cuda")) / theta).cpu().numpy()
         assert abs(c.mean()) < 5 * np.sqrt(1 / 3 / n) and abs((c**2).mean() - 1 / 3) < 5 * np.sqrt(4 / 45 / n)
-    # Marsaglia-Tsang acceptance, Eq. (28) region: p1 in (0.95, 1); a warp waits for its slowest lane
-    assert 1.0 <= lane < 1.06 and lane <= warp <= 2.2
+    # Marsaglia-Tsang acceptance rate, Eq. (28), k = kappa - 1/2: a lane makes 1/p1 trips on average
+    # ("3 + 2/p1 variates per particle on CPUs"); a warp waits for its slowest lane and
+    # makes mu_1(1 - p1, 32) trips, Eq. (30): 1.80, 1.60, 1.37, 1.10 at these four kappa.
+    k = kappa - 0.5
+    p1 = np.exp(k - 1.0 / 3.0) * special.gamma(k) / (np.sqrt(2 * np.pi) * (k - 1.0 / 3.0) ** (k - 0.5))
+    rho = 1.0 - p1
+    mu1 = 3.0 - (1.0 - rho) ** 32 - (1.0 - rho**2) ** 32
+    assert abs(mu1 - {1.6: 1.80, 2.0: 1.60, 3.0: 1.37, 10.0: 1.10}[kappa]) < 0.006
+    report(test="baseline_mt_trips", kappa=kappa, dtype=dtype, lane=lane, one_over_p1=1 / p1, warp=warp, mu1_eq30=mu1)
+    assert abs(lane - 1.0 / p1) <= 0.001, (lane, 1.0 / p1)
+    assert abs(warp - mu1) <= 0.01, (warp, mu1)
