@@ -132,6 +132,11 @@ def parse_args():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / baseline / cells extra timings")
+    ap.add_argument("--dist-backend", choices=["nccl", "gloo"], default="nccl",
+                    help="process group of the N>1 run; the data path has no collective, the group only carries the barrier, "
+                         "the max over ranks and the shard check (gloo: ranks may share one GPU, see --device-index)")
+    ap.add_argument("--device-index", type=int, default=None,
+                    help="CUDA device of this rank instead of LOCAL_RANK (to exercise the N>1 branch on a one-GPU box)")
     ap.add_argument("--pipe-rates", action="store_true",
                     help="print the kappagen_pipe_probe table (markdown) that profiles/r02_pipe_rates.md holds, and exit")
     ap.add_argument("--sweep", action="store_true",
@@ -287,9 +292,21 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    if args.device_index is not None:
+        local = args.device_index
     torch.cuda.set_device(local)
+    nccl = args.dist_backend == "nccl"
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if nccl:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
+
+    def max_over_ranks(x):
+        t = torch.tensor([x], dtype=torch.float64, device="cuda" if nccl else "cpu")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
     from paper_2602_05606_b200 import build as kbuild
     if rank == 0:
         kbuild.build()                                  # no-op when the in-tree library is up to date
@@ -321,11 +338,14 @@ def run_ours(args):
     total_ms, per_launch = time_launches(step, args.steps, 0, torch)
     barrier()
     clocks = sampler.stop()
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms)
     value = world * n * args.steps / (total_ms * 1e-3)
+    shards = None
+    if world > 1:                                       # what each rank's last timed step wrote, and from which offset
+        mine = {"rank": rank, "offset": ((args.steps - 1) * world + rank) * n, "device": local,
+                "vx_head": [float(v) for v in planes[0][:4].double().cpu()]}
+        shards = [None] * world
+        dist.all_gather_object(shards, mine)
     kern_ms = sum(per_launch) / len(per_launch)
 
     # ---- end to end through the C ABI with HOST buffers (device->host copies inside the timed region)
@@ -342,10 +362,7 @@ def run_ours(args):
         e2e_each.append(time.perf_counter() - t1)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * n * args.e2e_steps / float(te.item())
+    e2e_value = world * n * args.e2e_steps / max_over_ranks(e2e_s)
     checksum = float(host[0][:1024].double().abs().sum())                         # the host result is read
     del host, ws
 
@@ -367,6 +384,9 @@ def run_ours(args):
                     "value_at_median_step": world * n / sorted(e2e_each)[len(e2e_each) // 2]},
             "roofline": roofline_of(dtype, n, kern_ms, min(per_launch), max(per_launch), ceiling_ms),
         }
+        if shards is not None:
+            line["shards"] = shards
+            line["config"]["dist_backend"] = args.dist_backend
         if world == 1:                                   # the other dtype of the metric ("fp32/fp64"), same workload, this run
             other = "f64" if dtype == "f32" else "f32"
             op = tuple(torch.empty(n, dtype=torch.float64 if other == "f64" else torch.float32, device="cuda") for _ in range(3))
