@@ -16,31 +16,35 @@ namespace {
 
 typedef long double ld;
 
-// Continued fraction of the incomplete beta function (modified Lentz iteration, the classical
-// evaluation of I_x(a,b): DLMF 8.17.22).
-ld betacf(ld a, ld b, ld x) {
-    const ld tiny = 1e-4000L;
-    const ld qab = a + b, qap = a + 1.0L, qam = a - 1.0L;
-    ld c = 1.0L, d = 1.0L - qab * x / qap;
-    if (fabsl(d) < tiny) d = tiny;
-    d = 1.0L / d;
-    ld h = d;
-    for (int m = 1; m <= 2000; ++m) {
-        const ld m2 = 2.0L * m;
-        ld aa = m * (b - m) * x / ((qam + m2) * (a + m2));
-        d = 1.0L + aa * d; if (fabsl(d) < tiny) d = tiny;
-        c = 1.0L + aa / c; if (fabsl(c) < tiny) c = tiny;
-        d = 1.0L / d;
-        h *= d * c;
-        aa = -(a + m) * (qab + m) * x / ((a + m2) * (qap + m2));
-        d = 1.0L + aa * d; if (fabsl(d) < tiny) d = tiny;
-        c = 1.0L + aa / c; if (fabsl(c) < tiny) c = tiny;
-        d = 1.0L / d;
-        const ld del = d * c;
-        h *= del;
-        if (fabsl(del - 1.0L) < 1e-19L) break;
+// The continued fraction of the incomplete beta function, DLMF 8.17.22:
+//     I_x(a,b) = x^a (1-x)^b / (a B(a,b)) * 1 / (1 + d_1 / (1 + d_2 / (1 + ...))),
+//     d_{2m}   =  m (b - m) x / ((a + 2m - 1)(a + 2m)),
+//     d_{2m+1} = -(a + m)(a + b + m) x / ((a + 2m)(a + 2m + 1)).
+ld beta_cf_term(int j, ld a, ld b, ld x) {
+    const ld m = (ld)(j / 2);
+    if (j % 2 == 0) return m * (b - m) * x / ((a + 2.0L * m - 1.0L) * (a + 2.0L * m));
+    return -(a + m) * (a + b + m) * x / ((a + 2.0L * m) * (a + 2.0L * m + 1.0L));
+}
+
+// 1 / (1 + d_1 / (1 + d_2 / ...)) by the modified Lentz recurrence for f = b_0 + a_1/(b_1 + a_2/(b_2 + ...)) with every
+// b_j = 1 and a_j = d_j (DLMF 3.10(iii) names the method): C_j = 1 + d_j / C_{j-1}, D_j = 1 / (1 + d_j D_{j-1}),
+// f_j = f_{j-1} C_j D_j, from f_0 = C_0 = 1, D_0 = 0; a vanishing denominator is replaced by the smallest long double
+// that still inverts.  Converges fast for x < (a + 1) / (a + b + 2), which is how betainc_both() calls it.
+ld beta_cf(ld a, ld b, ld x) {
+    const ld floor_ld = 1e-4000L;
+    ld f = 1.0L, C = 1.0L, D = 0.0L;
+    for (int j = 1; j <= 4000; ++j) {
+        const ld dj = beta_cf_term(j, a, b, x);
+        ld den = 1.0L + dj * D;
+        if (fabsl(den) < floor_ld) den = floor_ld;
+        D = 1.0L / den;
+        C = 1.0L + dj / C;
+        if (fabsl(C) < floor_ld) C = floor_ld;
+        const ld step = C * D;
+        f *= step;
+        if (fabsl(step - 1.0L) < 1e-19L) break;
     }
-    return h;
+    return 1.0L / f;
 }
 
 // Regularized incomplete beta I_x(a,b) and its complement, each computed without cancellation.
@@ -50,10 +54,10 @@ void betainc_both(ld a, ld b, ld x, ld* I, ld* Ic) {
     const ld lnfront = lgammal(a + b) - lgammal(a) - lgammal(b) + a * logl(x) + b * log1pl(-x);
     const ld front = expl(lnfront);
     if (x < (a + 1.0L) / (a + b + 2.0L)) {
-        *I = front * betacf(a, b, x) / a;
+        *I = front * beta_cf(a, b, x) / a;
         *Ic = 1.0L - *I;
     } else {
-        *Ic = front * betacf(b, a, 1.0L - x) / b;
+        *Ic = front * beta_cf(b, a, 1.0L - x) / b;
         *I = 1.0L - *Ic;
     }
 }

@@ -1,4 +1,5 @@
-"""Full element-wise parity at FULL size for BASELINE.json configs[2], [3], [4] (C3 fp32 and fp64, C4, C5):
+"""Full element-wise parity at FULL size for BASELINE.json configs[1], [2], [3], [4] (C2's six kappa, C3 fp32 and fp64,
+C4, C5):
 every particle of the GPU output against the oracle, the oracle run over disjoint index ranges on all host
 cores (SURVEY.md section 8(c)-F "Coverage at scale": counter-based => trivially splittable).
 
@@ -96,6 +97,15 @@ def _check_sample(got, n, kappa, theta, seed, offset, dtype, name):
 
 @pytest.mark.parametrize("cfg", [wl.C3_F32, wl.C3_F64], ids=lambda c: c.name)
 def test_config3_every_particle(cfg):
+    got = kg.sample(cfg.n, cfg.kappa, cfg.theta, cfg.seed, cfg.offset, cfg.dtype)
+    torch.cuda.synchronize()
+    _check_sample(got, cfg.n, cfg.kappa, cfg.theta, cfg.seed, cfg.offset, cfg.dtype, cfg.name)
+
+
+@pytest.mark.parametrize("cfg", wl.C2, ids=lambda c: c.name)
+def test_config2_every_particle(cfg):
+    """configs[1]: 10^8 particles at each kappa of the paper's scan (1.6 ... 10), every particle (SURVEY.md section
+    8(c)-F: "Full element-wise parity for C1, C2"); the statistical side of this configuration is test_config2_gpu's."""
     got = kg.sample(cfg.n, cfg.kappa, cfg.theta, cfg.seed, cfg.offset, cfg.dtype)
     torch.cuda.synchronize()
     _check_sample(got, cfg.n, cfg.kappa, cfg.theta, cfg.seed, cfg.offset, cfg.dtype, cfg.name)
