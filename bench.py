@@ -76,7 +76,7 @@ def measured_peaks():
     return peak, which, mhz
 
 
-def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None):
+def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None, math_ms=None):
     """The roofline object of sample_kernel<dtype> from this run's CUDA-event time per launch.
     `bound`/`achieved`/`peak`/`frac` name the pipe that actually limits the kernel (both dtypes: an arithmetic pipe,
     "alu"): algorithmic pipe operations per second against the pipe's issue rate.  The north_star's own figures stay
@@ -120,6 +120,13 @@ def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None):
         r["ceiling"] = {"kernel": "philox_planes_kernel (S1 + S6 only, 12 B/particle)", "kernel_ms": ceiling_ms,
                         "particles_per_s": n / (ceiling_ms * 1e-3)}
         r["frac_of_ceiling"] = ceiling_ms / kern_ms
+    if math_ms is not None:
+        cyc = lambda ms: ms * 1e-3 * mhz * 1e6 * N_SM * 4 * 32 / n
+        r["math_only"] = {"kernel": "math_planes_kernel (S2-S6 + stores, words from one IMAD each)", "kernel_ms": math_ms,
+                          "particles_per_s": n / (math_ms * 1e-3), "cycles_per_32_particles": cyc(math_ms),
+                          "sampler_cycles_per_32_particles": cyc(kern_ms), "philox_share_of_sampler_time": 1.0 - math_ms / kern_ms}
+        if dtype == "f64":
+            r["math_only"]["fp64_pipe_frac"] = ops * n / (math_ms * 1e-3) / 1e9 / alu_peak
     return r
 
 
@@ -138,7 +145,7 @@ def parse_args():
     ap.add_argument("--device-index", type=int, default=None,
                     help="CUDA device of this rank instead of LOCAL_RANK (to exercise the N>1 branch on a one-GPU box)")
     ap.add_argument("--pipe-rates", action="store_true",
-                    help="print the kappagen_pipe_probe table (markdown) that profiles/r02_pipe_rates.md holds, and exit")
+                    help="print the kappagen_pipe_probe table (markdown) that profiles/r03_pipe_rates.md holds, and exit")
     ap.add_argument("--sweep", action="store_true",
                     help="also time kappagen_sample over 1e6 ... 2^30 particles and kappa 1.6 ... 10 (extras.sweep)")
     return ap.parse_args()
@@ -373,6 +380,9 @@ def run_ours(args):
             wp = tuple(p.view(torch.int32) for p in planes)
             _, cms = time_launches(lambda s: kg.philox_planes(n, SEED, s * n, out=wp, stream=stream), 10, 3, torch)
             ceiling_ms = sum(cms) / len(cms)
+        # ... and with S1 stripped instead: the math and the stores on affine words (kappagen_math_planes)
+        _, mms = time_launches(lambda s: kg.math_planes(n, KAPPA, THETA, s * n, dtype, out=planes, stream=stream), 10, 3, torch)
+        math_ms = sum(mms) / len(mms)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -382,7 +392,7 @@ def run_ours(args):
                     "steps": args.e2e_steps, "api": "kappagen_sample_host_ws (pinned host planes, caller's staging workspace and streams)",
                     "checksum": checksum, "ms_per_step": [round(1e3 * t, 3) for t in e2e_each],
                     "value_at_median_step": world * n / sorted(e2e_each)[len(e2e_each) // 2]},
-            "roofline": roofline_of(dtype, n, kern_ms, min(per_launch), max(per_launch), ceiling_ms),
+            "roofline": roofline_of(dtype, n, kern_ms, min(per_launch), max(per_launch), ceiling_ms, math_ms),
         }
         if shards is not None:
             line["shards"] = shards
@@ -392,7 +402,8 @@ def run_ours(args):
             op = tuple(torch.empty(n, dtype=torch.float64 if other == "f64" else torch.float32, device="cuda") for _ in range(3))
             _, oms = time_launches(lambda s: kg.sample(n, KAPPA, THETA, SEED, s * n, other, out=op, stream=stream), 20, 3, torch)
             k = sum(oms) / len(oms)
-            line["roofline_" + other] = roofline_of(other, n, k, min(oms), max(oms))
+            _, mms = time_launches(lambda s: kg.math_planes(n, KAPPA, THETA, s * n, other, out=op, stream=stream), 10, 3, torch)
+            line["roofline_" + other] = roofline_of(other, n, k, min(oms), max(oms), None, sum(mms) / len(mms))
             line["value_" + other] = n / (k * 1e-3)
             del op
         if world == 1 and not args.no_extras:
@@ -510,21 +521,22 @@ def pipe_rates():
     from paper_2602_05606_b200 import kappagen as kg
     if not torch.cuda.is_available():
         raise SystemExit("--pipe-rates needs a CUDA device")
-    print("| mix | instructions per iteration | w=1 | w=2 | w=4 | w=8 | sum of single-kind costs at w=8 |")
-    print("|---|---|---|---|---|---|---|")
+    ws = (1, 2, 3, 4, 8)                                  # 3 = the double sampler's warps per scheduler (one block of 384)
+    print("| mix | instructions per iteration | " + " | ".join("w=%d" % w for w in ws) + " | sum of single-kind costs at w=8 |")
+    print("|---|---|" + "---|" * (len(ws) + 1))
     single = {}
     rows = []
     for mix in range(kg.pipe_probe_count()):
-        cyc = [kg.pipe_probe(mix, w, 2048) for w in (1, 2, 4, 8)]
+        cyc = [kg.pipe_probe(mix, w, 2048) for w in ws]
         counts = cyc[0][1]
         if len(counts) == 1:
             (kind, cnt), = counts.items()
-            single[kind] = cyc[3][0] / cnt
+            single[kind] = cyc[-1][0] / cnt
         rows.append((mix, counts, [c[0] for c in cyc]))
     for mix, counts, c in rows:
         add = sum(single.get(k, float("nan")) * v for k, v in counts.items())
-        print("| %d | %s | %.1f | %.1f | %.1f | %.1f | %.1f |" % (mix, " + ".join("%d %s" % (v, k) for k, v in counts.items()),
-                                                               c[0], c[1], c[2], c[3], add))
+        print("| %d | %s | %s | %.1f |" % (mix, " + ".join("%d %s" % (v, k) for k, v in counts.items()),
+                                          " | ".join("%.1f" % x for x in c), add))
     print()
     print("cycles per warp instruction per scheduler at w=8 (loop overhead of ~3 instructions per iteration included): " +
           ", ".join("%s %.2f" % (k, v) for k, v in single.items()))

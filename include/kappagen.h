@@ -194,6 +194,18 @@ int kappagen_load_cells(int64_t ncell, int32_t ppc, const void* kappa, const voi
 int kappagen_philox_planes(int64_t n, uint64_t seed, uint64_t offset,
                            uint32_t* w0, uint32_t* w1, uint32_t* w2, void* stream);
 
+/* Measurement hook, the counterpart of kappagen_philox_planes: steps S2-S6 alone.  The sampler's whole-tile body for
+ * `dtype` (same device functions, tile shape, launch bounds and 128-bit streaming stores) with step S1 replaced by one
+ * 32-bit multiply-add per word: particle g = offset + i takes
+ *     w_k = lo32(g) * M_k + A_k  (mod 2^32),   M = (0x9E3779B1, 0x85EBCA77, 0xC2B2AE3D),  A = (0x7F4A7C15, 0x165667B1, 0x27D4EB2F)
+ * and writes the velocity kappagen_velocity_of_words_tile gives for (w_0, w_1, w_2) (bit-identical; flags = 0).  Its
+ * rate is what the math and the stores cost when the random words are almost free: the ceiling of kappagen_sample from
+ * the side opposite to kappagen_philox_planes (bench.py times both).  NOT a random-number generator.
+ * vx, vy, vz: device, [n] elements of `dtype`, 16-byte aligned (KAPPAGEN_EALIGN otherwise).  kappa, theta: as
+ * kappagen_sample. */
+int kappagen_math_planes(int64_t n, double kappa, double theta, uint64_t offset, int dtype,
+                         void* vx, void* vy, void* vz, void* stream);
+
 /* Measurement hook: issue-rate probe behind the "alu" rooflines of DESIGN.md section 5 and profiles/r02_pipe_rates.md.
  * Runs a register-only loop of a fixed instruction mix (eight independent chains per kind: IMAD.WIDE.U32, LOP3, FFMA2,
  * MUFU.EX2, DFMA, IMAD) on every SM with `warps_per_scheduler` warps per SM sub-partition and reports the mean

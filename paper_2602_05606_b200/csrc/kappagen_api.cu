@@ -895,6 +895,41 @@ extern "C" int kappagen_philox_planes(int64_t n, uint64_t seed, uint64_t offset,
     return KAPPAGEN_OK;
 }
 
+template <typename T, bool FOLD>
+static int launch_math_planes(int64_t n, uint64_t offset, const Coef<T>& C, T* vx, T* vy, T* vz, cudaStream_t st) {
+    constexpr int threads = TileTraits<T>::threads;
+    constexpr int64_t tile = (int64_t)threads * (16 / sizeof(T)) * TileTraits<T>::groups;
+    int grid = 0, rc;
+    if ((rc = grid_for<math_planes_kernel<T, FOLD>>((n + tile - 1) / tile, &grid, threads)) != KAPPAGEN_OK) return rc;
+    math_planes_kernel<T, FOLD><<<grid, threads, 0, st>>>(n, offset, C, vx, vy, vz);
+    KG_CUDA(cudaGetLastError());
+    return KAPPAGEN_OK;
+}
+
+extern "C" int kappagen_math_planes(int64_t n, double kappa, double theta, uint64_t offset, int dtype, void* vx, void* vy,
+                                    void* vz, void* stream) {
+    const char* fn = "kappagen_math_planes";
+    bool vec = false;
+    int rc = check_planes(fn, n, dtype, vx, vy, vz, &vec);
+    if (rc != KAPPAGEN_OK) return rc;
+    if (!domain_ok(kappa, theta)) {
+        set_error("%s: need finite kappa > 3/2 and theta >= 0 (got kappa = %g, theta = %g)", fn, kappa, theta);
+        return KAPPAGEN_EINVAL;
+    }
+    if (n == 0) return KAPPAGEN_OK;
+    if (!vec) {
+        set_error("%s: the planes must be 16-byte aligned (this hook has the vector-store path only)", fn);
+        return KAPPAGEN_EALIGN;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == KAPPAGEN_F64)
+        return launch_math_planes<double, false>(n, offset, host_coef_f64(kappa, theta), (double*)vx, (double*)vy, (double*)vz, st);
+    const bool fold = theta_folds(theta);
+    const Coef<float> C = host_coef_f32(kappa, theta, fold);
+    return fold ? launch_math_planes<float, true>(n, offset, C, (float*)vx, (float*)vy, (float*)vz, st)
+                : launch_math_planes<float, false>(n, offset, C, (float*)vx, (float*)vy, (float*)vz, st);
+}
+
 extern "C" int kappagen_pipe_probe_count(void) { return kPipeMixCount; }
 
 extern "C" int kappagen_pipe_probe(int mix, int warps_per_scheduler, int iters, double* cycles_per_iter, int* counts) {

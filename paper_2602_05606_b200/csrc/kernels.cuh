@@ -721,6 +721,68 @@ philox_planes_kernel(int64_t n, uint64_t offset, const __grid_constant__ PhiloxK
     }
 }
 
+// ---------------------------------------------------------------- kappagen_math_planes (measurement hook)
+// The other side of kappagen_philox_planes: steps S2-S6 of the sampler's whole-tile body -- the same words_to_velocities,
+// the same tile shape, launch bounds and 128-bit streaming stores -- with S1 (Philox) replaced by one 32-bit
+// multiply-add per word, w_k = lo32(g) * kMathPlanesMul<k> + kMathPlanesAdd<k>: what the math and the stores cost
+// when the random words are (almost) free.  Not a generator: the words are a fixed affine map of the index.
+constexpr uint32_t kMathPlanesMul0 = 0x9E3779B1u, kMathPlanesMul1 = 0x85EBCA77u, kMathPlanesMul2 = 0xC2B2AE3Du;
+constexpr uint32_t kMathPlanesAdd0 = 0x7F4A7C15u, kMathPlanesAdd1 = 0x165667B1u, kMathPlanesAdd2 = 0x27D4EB2Fu;
+
+template <int G>
+__device__ __forceinline__ void affine_words(uint32_t lo, uint32_t (&w0)[G], uint32_t (&w1)[G], uint32_t (&w2)[G], uint32_t (&w3)[G]) {
+#pragma unroll
+    for (int e = 0; e < G; ++e) {
+        const uint32_t g = lo + (uint32_t)e;
+        w0[e] = g * kMathPlanesMul0 + kMathPlanesAdd0;
+        w1[e] = g * kMathPlanesMul1 + kMathPlanesAdd1;
+        w2[e] = g * kMathPlanesMul2 + kMathPlanesAdd2;
+        w3[e] = 0u;
+    }
+}
+
+template <typename T, bool FOLD>
+__global__ void __launch_bounds__(TileTraits<T>::threads, TileTraits<T>::minb)
+math_planes_kernel(int64_t n, uint64_t offset, const __grid_constant__ Coef<T> C, T* __restrict__ vx, T* __restrict__ vy,
+                   T* __restrict__ vz) {
+    constexpr int G = 16 / sizeof(T);
+    constexpr int NG = TileTraits<T>::groups;
+    constexpr int kT = TileTraits<T>::threads;
+    constexpr int64_t kTile = (int64_t)kT * G * NG;
+    math_tables_init<T>();
+    for (int64_t base = (int64_t)blockIdx.x * kTile; base < n; base += (int64_t)gridDim.x * kTile) {
+        const uint32_t lo_first = (uint32_t)(offset + (uint64_t)base) + threadIdx.x * (uint32_t)G;
+        if (base + kTile <= n) {
+            T ox[NG][G], oy[NG][G], oz[NG][G];
+#pragma unroll
+            for (int j = 0; j < NG; ++j) {
+                uint32_t w0[G], w1[G], w2[G], w3[G];
+                affine_words<G>(lo_first + (uint32_t)(j * (kT * G)), w0, w1, w2, w3);
+                words_to_velocities<FOLD, false>(w0, w1, w2, w3, C, ox[j], oy[j], oz[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < NG; ++j) {
+                const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+                store_group(vx + i, ox[j]);
+                store_group(vy + i, oy[j]);
+                store_group(vz + i, oz[j]);
+            }
+            continue;
+        }
+#pragma unroll 1
+        for (int j = 0; j < NG; ++j) {
+            const int64_t i = base + (int64_t)j * (kT * G) + (int64_t)threadIdx.x * G;
+            if (i < n) {
+                uint32_t w0[G], w1[G], w2[G], w3[G];
+                T ox[G], oy[G], oz[G];
+                affine_words<G>(lo_first + (uint32_t)(j * (kT * G)), w0, w1, w2, w3);
+                words_to_velocities<FOLD, false>(w0, w1, w2, w3, C, ox, oy, oz);
+                store_planes<T, false, G>(i, n, vx, vy, vz, ox, oy, oz);
+            }
+        }
+    }
+}
+
 // S2-S6 on caller-chosen words through the code sample_kernel<T> ships: every thread takes the NG groups of
 // a tile in one straight line through words_to_velocities (float: the packed pairs of math_f32x2.cuh; double:
 // the 2 NG interleaved chains), exactly as the whole-tile path instantiates them -- only the source of the

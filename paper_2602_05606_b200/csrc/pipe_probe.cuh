@@ -38,6 +38,11 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(int iters, uint32_t se
     constexpr int kMax = NW > NL ? (NW > NP ? NW : NP) : (NL > NP ? NL : NP);
     constexpr int kMax2 = NM > ND ? (NM > NI ? NM : NI) : (ND > NI ? ND : NI);
     constexpr int kRounds = ((kMax > kMax2 ? kMax : kMax2) + 7) / 8;
+    // Counts that are multiples of 8 fill whole rounds from the front (mixes 0-20, as measured in round 2).  Any other
+    // count -- the kernels' exact proportions, mixes 21 on -- is spread evenly over the 8 * kRounds slots of the body.
+    constexpr bool kSpread = (NW % 8 != 0) || (NL % 8 != 0) || (NP % 8 != 0) || (NM % 8 != 0) || (ND % 8 != 0) || (NI % 8 != 0);
+    constexpr int kSlots = 8 * kRounds;
+#define KG_PROBE_EMIT(N, s) (kSpread ? (((s) + 1) * (N) / kSlots > (s) * (N) / kSlots) : ((s) < (N)))
     const long long t0 = clock64();
 #pragma unroll 1
     for (int it = 0; it < iters; ++it) {
@@ -45,21 +50,22 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(int iters, uint32_t se
         for (int r = 0; r < kRounds; ++r) {
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-                if (r * 8 + k < NW) {
+                if (KG_PROBE_EMIT(NW, r * 8 + k)) {
                     unsigned long long q;
                     uint32_t lo, hi;
                     asm volatile("mul.wide.u32 %0, %1, 0xD2511F53;" : "=l"(q) : "r"(w[k]));
                     asm volatile("mov.b64 {%0,%1}, %2;" : "=r"(lo), "=r"(hi) : "l"(q));
                     w[k] = hi;
                 }
-                if (r * 8 + k < NL) asm volatile("lop3.b32 %0, %0, %1, 0x9E3779B9, 0x96;" : "+r"(l[k]) : "r"(l[(k + 1) & 7]));
-                if (r * 8 + k < NP) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(p[k]) : "l"(pa), "l"(pb));
-                if (r * 8 + k < NM) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(m[k]));
-                if (r * 8 + k < ND) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[k]) : "d"(da), "d"(db));
-                if (r * 8 + k < NI) asm volatile("mad.lo.u32 %0, %0, 0xD2511F53, %1;" : "+r"(im[k]) : "r"(seed));
+                if (KG_PROBE_EMIT(NL, r * 8 + k)) asm volatile("lop3.b32 %0, %0, %1, 0x9E3779B9, 0x96;" : "+r"(l[k]) : "r"(l[(k + 1) & 7]));
+                if (KG_PROBE_EMIT(NP, r * 8 + k)) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(p[k]) : "l"(pa), "l"(pb));
+                if (KG_PROBE_EMIT(NM, r * 8 + k)) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(m[k]));
+                if (KG_PROBE_EMIT(ND, r * 8 + k)) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[k]) : "d"(da), "d"(db));
+                if (KG_PROBE_EMIT(NI, r * 8 + k)) asm volatile("mad.lo.u32 %0, %0, 0xD2511F53, %1;" : "+r"(im[k]) : "r"(seed));
             }
         }
     }
+#undef KG_PROBE_EMIT
     const long long t1 = clock64();
     uint32_t acc = 0u;
 #pragma unroll
@@ -81,6 +87,10 @@ constexpr PipeMix kPipeMixes[] = {
     {8, 0, 0, 4, 0, 0},  {8, 0, 0, 0, 8, 0},  {8, 0, 0, 0, 16, 0}, {4, 0, 0, 0, 16, 0}, {0, 8, 0, 0, 16, 0},  // 10-14
     {0, 0, 0, 0, 16, 8}, {0, 16, 8, 4, 0, 0}, {8, 16, 8, 4, 0, 0}, {8, 16, 0, 4, 0, 0}, {4, 8, 0, 2, 16, 0},  // 15-19
     {0, 8, 0, 2, 16, 0},                                                                                      // 20
+    // 21: the double sampler's own instruction mix per particle (cuobjdump -sass, whole-tile body of
+    // sample_kernel<double,1,0,0>, profiles/r03_fp64_limit.md): 85 FP64, 18 wide multiplies, 56 ALU-pipe, 6 MUFU, 9 IMAD;
+    // 22: the same without the wide multiplies (the mix of kappagen_math_planes); 23: FP64 + ALU only
+    {18, 56, 0, 6, 85, 9}, {0, 56, 0, 6, 85, 9}, {0, 56, 0, 0, 85, 0},                                        // 21-23
 };
 constexpr int kPipeMixCount = (int)(sizeof(kPipeMixes) / sizeof(kPipeMixes[0]));
 

@@ -62,6 +62,7 @@ def lib() -> ctypes.CDLL:
         L.kappagen_sample_host_workspace_bytes.restype = sz
         L.kappagen_load_cells.argtypes = [i64, i32, vp, vp, vp, i64, vp, i64, u64, u64, ci, vp, vp, sz, vp]
         L.kappagen_philox_planes.argtypes = [i64, u64, u64, vp, vp, vp, vp]
+        L.kappagen_math_planes.argtypes = [i64, f64, f64, u64, ci, vp, vp, vp, vp]
         L.kappagen_pipe_probe.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ci)]
         L.kappagen_baseline_mt.argtypes = [i64, f64, f64, u64, u64, ci, vp, vp, vp, vp, vp]
         L.kappagen_words.argtypes = [i64, u64, u64, vp, vp, vp, vp]
@@ -75,7 +76,7 @@ def lib() -> ctypes.CDLL:
                      "kappagen_sample_cells", "kappagen_sample_cells_static", "kappagen_sample_cells_moments", "kappagen_sample_host", "kappagen_baseline_mt",
                      "kappagen_words", "kappagen_velocity_of_words", "kappagen_params", "kappagen_version",
                      "kappagen_words_tile", "kappagen_velocity_of_words_tile", "kappagen_sample_host_ws",
-                     "kappagen_load_cells", "kappagen_cells_prepare", "kappagen_sample_cells_prepared", "kappagen_philox_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
+                     "kappagen_load_cells", "kappagen_cells_prepare", "kappagen_sample_cells_prepared", "kappagen_philox_planes", "kappagen_math_planes", "kappagen_pipe_probe", "kappagen_pipe_probe_count"):
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -343,6 +344,18 @@ def philox_planes(n: int, seed: int, offset: int = 0, out=None, stream=None, dev
     _same_device(*out)
     _check(lib().kappagen_philox_planes(n, seed, offset, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), _stream(stream)))
     return out
+
+
+MATH_PLANES_MUL = (0x9E3779B1, 0x85EBCA77, 0xC2B2AE3D)       # kappagen_math_planes: w_k = lo32(g) * MUL[k] + ADD[k] mod 2^32
+MATH_PLANES_ADD = (0x7F4A7C15, 0x165667B1, 0x27D4EB2F)
+
+
+def math_planes(n: int, kappa: float, theta: float, offset: int = 0, dtype="f32", out=None, stream=None, device="cuda"):
+    """kappagen_math_planes: S2-S6 + stores on affine words of the index (the sampler's ceiling from the math side)."""
+    code = _dtype_code(dtype)
+    vx, vy, vz = _planes(n, code, out, device)
+    _check(lib().kappagen_math_planes(n, kappa, theta, offset, code, vx.data_ptr(), vy.data_ptr(), vz.data_ptr(), _stream(stream)))
+    return vx, vy, vz
 
 
 PIPE_KINDS = ("IMAD.WIDE.U32", "LOP3", "FFMA2", "MUFU.EX2", "DFMA", "IMAD")
