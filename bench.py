@@ -46,19 +46,25 @@ def load_ncu():
 
 
 NCU_CAPTURE, NCU_TRAFFIC_BYTES, NCU_PIPE_PCT = load_ncu()
+
+
+def probe_mix_cycles():
+    """Cycles per 32 particles of a dependency-free, memory-free loop with the double sampler's exact instruction mix at
+    its 3 warps per scheduler (kappagen_pipe_probe mix 21, profiles/r03_pipe_rates.md via r03_ncu.json)."""
+    with open(os.path.join(ROOT, "profiles", "r03_ncu.json")) as f:
+        return float(json.load(f)["pipe_probe"]["double_sampler_mix"]["cycles_per_iteration"]["w3"])
 # Algorithmic work per particle on the arithmetic pipes (DESIGN.md section 5; instruction counts from cuobjdump -sass,
-# rates from kappagen_pipe_probe = profiles/r02_pipe_rates.md), in thread-operations per clock per SM:
+# rates from kappagen_pipe_probe = profiles/r03_pipe_rates.md), in thread-operations per clock per SM:
 #   f32: Philox4x32-10 with counter words 2,3 = 0 needs 19 32x32->64-bit multiplies; IMAD.WIDE issues at a quarter of
 #        the 128-lane FMA rate (probe: 4.1 cycles per warp instruction per scheduler) -> 32 /clk/SM.
 #   f64: the double chain is 85 FP64 instructions (DFMA/DMUL/DADD/DSETP) per particle; 64 /clk/SM.  On sm_100 the FP64
-#        pipe and the FMA-heavy pipe (Philox's IMAD.WIDE) overlap only in part; their issue cycles per 32 particles sum
-#        to 85 x 2.03 + 18.2 x 4.14 + 9 x 2 scheduler cycles.
+#        pipe and the FMA-heavy pipe (Philox's IMAD.WIDE) overlap only in part: a loop of the kernel's exact mix, free of
+#        dependencies and memory, takes 259.3 cycles per 32 particles (profiles/r03_fp64_limit.md), the kernel 288.
 ALU_WORK = {"f32": (19, 32, "G mul.wide.u32/s", "fmaheavy (IMAD.WIDE.U32, quarter rate)"),
             "f64": (85, 64, "G FP64 instr/s", "fp64 (DFMA/DMUL/DADD)")}
 # What the SASS executes per particle on that pipe: the shared Philox head per tile leaves 18.1 of the 19 algorithmic
 # multiplies (17.1 IMAD.WIDE + 1 IMAD.HI, profiles/r02_fp32_limit.md); the double chain executes its 85.
 ALU_EXECUTED = {"f32": 18.1, "f64": 85.0}
-F64_SHARED_PORT_CYCLES = 85 * 2.03 + 18.2 * 4.14 + 9 * 2.0    # per 32 particles per scheduler: FP64 + IMAD.WIDE + IMAD/MOV
 TARGETS = {"f32": ("hbm", 0.80), "f64": ("alu", 0.70)}         # BASELINE.json north_star, last sentence
 BOUND = {"f32": "alu", "f64": "alu"}                           # the measured limiter of each kernel (ncu pipe figures)
 
@@ -92,7 +98,7 @@ def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None, math_ms=
     alu_peak = N_SM * per_clk * mhz * 1e6 / 1e9
     alu = {"achieved": ops * rate / 1e9, "peak": alu_peak, "unit": alu_unit, "pipe": pipe,
            "algorithmic_ops_per_particle": ops,
-           "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5, profiles/r02_pipe_rates.md)" % (N_SM, per_clk, mhz)}
+           "peak_source": "%d SMs x %d thread-ops/clk/SM x %.0f MHz (DESIGN.md section 5, profiles/r03_pipe_rates.md)" % (N_SM, per_clk, mhz)}
     alu["frac"] = alu["achieved"] / alu_peak
     alu["executed_ops_per_particle"] = ALU_EXECUTED[dtype]
     alu["frac_executed"] = alu["frac"] * ALU_EXECUTED[dtype] / ops
@@ -111,11 +117,13 @@ def roofline_of(dtype, n, kern_ms, kern_min, kern_max, ceiling_ms=None, math_ms=
                            "(target), frac_of_ceiling the same kernel with steps S2-S5 stripped (kappagen_philox_planes)")
     else:
         cyc = kern_ms * 1e-3 * mhz * 1e6 * N_SM * 4 * 32 / n           # scheduler cycles per 32 particles
-        r["shared_port"] = {"cycles_per_32_particles": cyc, "fp64_plus_fmaheavy_cycles": F64_SHARED_PORT_CYCLES,
-                            "frac": F64_SHARED_PORT_CYCLES / cyc,
-                            "note": "model: FP64 and FMA-heavy (IMAD.WIDE, IMAD) instructions overlap only in part on sm_100 "
-                                    "(profiles/r02_pipe_rates.md, mixes 11-15; ncu: fp64 + fmaheavy busy fractions add up to 92 %); "
-                                    "this is the sum of their issue cycles per 32 particles over the elapsed cycles"}
+        bound = probe_mix_cycles()
+        r["mix_bound"] = {"cycles_per_32_particles": cyc, "probe_mix_cycles": bound, "frac": bound / cyc,
+                          "fp64_pipe_frac_at_bound": ops * 32 / (per_clk / 4) / bound,
+                          "note": "kappagen_pipe_probe mix 21 = this kernel's instruction mix per particle (85 FP64, 18 wide "
+                                  "multiplies, 56 ALU, 6 MUFU, 9 IMAD) without dependencies or memory, at the kernel's 3 warps per "
+                                  "scheduler: the bound of ANY schedule of this mix (profiles/r03_fp64_limit.md); frac = how close "
+                                  "the kernel is to it"}
     if ceiling_ms is not None:
         r["ceiling"] = {"kernel": "philox_planes_kernel (S1 + S6 only, 12 B/particle)", "kernel_ms": ceiling_ms,
                         "particles_per_s": n / (ceiling_ms * 1e-3)}

@@ -206,7 +206,7 @@ int kappagen_philox_planes(int64_t n, uint64_t seed, uint64_t offset,
 int kappagen_math_planes(int64_t n, double kappa, double theta, uint64_t offset, int dtype,
                          void* vx, void* vy, void* vz, void* stream);
 
-/* Measurement hook: issue-rate probe behind the "alu" rooflines of DESIGN.md section 5 and profiles/r02_pipe_rates.md.
+/* Measurement hook: issue-rate probe behind the "alu" rooflines of DESIGN.md section 5 and profiles/r03_pipe_rates.md.
  * Runs a register-only loop of a fixed instruction mix (eight independent chains per kind: IMAD.WIDE.U32, LOP3, FFMA2,
  * MUFU.EX2, DFMA, IMAD) on every SM with `warps_per_scheduler` warps per SM sub-partition and reports the mean
  * cycles per loop iteration per warp (clock64 around the loop, averaged over blocks).

@@ -13,7 +13,7 @@
 //
 // Written for the FP64 pipe of sm_100 (64 DFMA/clk/SM): 85 FP64 instructions per particle instead of
 // libdevice's ~200, and no divergent slow paths.  On sm_100 the FP64 pipe and the FMA-heavy pipe (IMAD,
-// IMAD.WIDE, IMAD.MOV) do not overlap in time (profiles/r02_pipe_rates.md), so every instruction of either
+// IMAD.WIDE, IMAD.MOV) do not overlap in time (profiles/r03_pipe_rates.md), so every instruction of either
 // kind counts against the same budget; the choices below follow from that.
 //   * integer -> double without a conversion instruction: 1 + w 2^-32 is the register pair
 //     ((w >> 12) + 0x3ff00000, w << 20), two ALU instructions and no move; one exact DADD re-centres it.

@@ -1,6 +1,6 @@
 // pipe_probe.cuh -- issue-rate probe of the sm_100 pipes the kappagen kernels are bound by (kappagen_pipe_probe,
 // include/kappagen.h).  Not on the hot path: it is the tracked source of the per-instruction cycle figures that
-// DESIGN.md section 5 and profiles/r02_pipe_rates.md quote (the "alu" roofline peaks of bench.py).
+// DESIGN.md section 5 and profiles/r03_pipe_rates.md quote (the "alu" roofline peaks of bench.py).
 //
 // Each mix is a register-only loop body of N instructions per kind, eight independent dependency chains per kind so
 // that latency never binds; inline PTX, one SASS instruction each:
@@ -16,7 +16,7 @@
 
 namespace kappagen {
 
-template <int NW, int NL, int NP, int NM, int ND, int NI>
+template <int NW, int NL, int NP, int NM, int ND, int NI, bool kSpread>
 __global__ void __launch_bounds__(1024) pipe_probe_kernel(int iters, uint32_t seed, uint32_t* sink, long long* cycles) {
     uint32_t w[8], l[8], im[8];
     float m[8];
@@ -38,9 +38,8 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(int iters, uint32_t se
     constexpr int kMax = NW > NL ? (NW > NP ? NW : NP) : (NL > NP ? NL : NP);
     constexpr int kMax2 = NM > ND ? (NM > NI ? NM : NI) : (ND > NI ? ND : NI);
     constexpr int kRounds = ((kMax > kMax2 ? kMax : kMax2) + 7) / 8;
-    // Counts that are multiples of 8 fill whole rounds from the front (mixes 0-20, as measured in round 2).  Any other
-    // count -- the kernels' exact proportions, mixes 21 on -- is spread evenly over the 8 * kRounds slots of the body.
-    constexpr bool kSpread = (NW % 8 != 0) || (NL % 8 != 0) || (NP % 8 != 0) || (NM % 8 != 0) || (ND % 8 != 0) || (NI % 8 != 0);
+    // kSpread = false (mixes 0-20, laid out as in round 2): each kind fills the body's slots from the front.  kSpread = true
+    // (the kernels' exact proportions, mixes 21 on): each kind is spread evenly over the 8 * kRounds slots of the body.
     constexpr int kSlots = 8 * kRounds;
 #define KG_PROBE_EMIT(N, s) (kSpread ? (((s) + 1) * (N) / kSlots > (s) * (N) / kSlots) : ((s) < (N)))
     const long long t0 = clock64();
@@ -78,6 +77,7 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(int iters, uint32_t se
 
 struct PipeMix {
     int wide, lop3, ffma2, mufu, dfma, imad;
+    bool spread = false;
 };
 // The table kappagen_pipe_probe indexes.  Single kinds first (the pipe rates), then pairs (which pipes overlap),
 // then the kernels' own proportions.
@@ -90,7 +90,7 @@ constexpr PipeMix kPipeMixes[] = {
     // 21: the double sampler's own instruction mix per particle (cuobjdump -sass, whole-tile body of
     // sample_kernel<double,1,0,0>, profiles/r03_fp64_limit.md): 85 FP64, 18 wide multiplies, 56 ALU-pipe, 6 MUFU, 9 IMAD;
     // 22: the same without the wide multiplies (the mix of kappagen_math_planes); 23: FP64 + ALU only
-    {18, 56, 0, 6, 85, 9}, {0, 56, 0, 6, 85, 9}, {0, 56, 0, 0, 85, 0},                                        // 21-23
+    {18, 56, 0, 6, 85, 9, true}, {0, 56, 0, 6, 85, 9, true}, {0, 56, 0, 0, 85, 0, true},                                        // 21-23
 };
 constexpr int kPipeMixCount = (int)(sizeof(kPipeMixes) / sizeof(kPipeMixes[0]));
 
@@ -98,7 +98,7 @@ typedef void (*PipeProbeFn)(int, uint32_t, uint32_t*, long long*);
 template <int I> struct PipeProbeTable {
     static void fill(PipeProbeFn* t) {
         constexpr PipeMix M = kPipeMixes[I];
-        t[I] = pipe_probe_kernel<M.wide, M.lop3, M.ffma2, M.mufu, M.dfma, M.imad>;
+        t[I] = pipe_probe_kernel<M.wide, M.lop3, M.ffma2, M.mufu, M.dfma, M.imad, M.spread>;
         PipeProbeTable<I + 1>::fill(t);
     }
 };

@@ -23,7 +23,12 @@ def test_roofline_objects_follow_from_the_kernel_time():
     assert r64["bound"] == "alu" and r64["frac"] == r64["frac_pipe"]
     assert math.isclose(r64["frac_pipe"], 85 * n / 2.07e-3 / (148 * 64 * mhz * 1e6), rel_tol=1e-12)
     assert math.isclose(r64["frac_hbm"], 24 * n / 2.07e-3 / 1e9 / peak, rel_tol=1e-12)
-    assert 0.5 < r64["shared_port"]["frac"] < 1.2 and "ceiling" not in r64
+    cyc = 2.07e-3 * mhz * 1e6 * 148 * 4 * 32 / n
+    assert math.isclose(r64["mix_bound"]["frac"], 259.3 / cyc, rel_tol=1e-12) and "ceiling" not in r64
+    assert math.isclose(r64["mix_bound"]["fp64_pipe_frac_at_bound"], 85 * 2 / 259.3, rel_tol=1e-12)   # 2 cycles per FP64 warp instruction
+    r64m = bench.roofline_of("f64", n, 2.07, 2.06, 2.10, None, 1.64)
+    assert math.isclose(r64m["math_only"]["fp64_pipe_frac"], r64["frac_pipe"] * 2.07 / 1.64, rel_tol=1e-12)
+    assert math.isclose(r64m["math_only"]["philox_share_of_sampler_time"], 1 - 1.64 / 2.07, rel_tol=1e-12)
     for r in (r32, r64):
         for key in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel_ms", "ncu"):
             assert key in r
